@@ -1,0 +1,117 @@
+"""oracle -- CPU oracle for the X-engine (ctypes binding over xcorr_oracle.c).
+
+TEST INFRASTRUCTURE: only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this
+package.  The product package never does (tests/test_independence.py checks).
+
+All arithmetic is in ``xcorr_oracle.c`` (read its header for the passages it
+follows: PAPER.md:47, :53, :84, :107, :115).  This file only marshals numpy
+arrays.  Parity status: every function below is pinned by
+``tests/test_oracle_pins.py`` (P1-P9, tests/golden/); none is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "xcorr_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+class OracleOverflow(ArithmeticError):
+    """A sum does not fit int32 (oracle refuses rather than wrap)."""
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2, no fused multiply-add contraction (Im V_ii must be exactly 0 in float64)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = f"{_LIB}.{os.getpid()}.tmp"
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+             "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        L, I, P = ctypes.c_long, ctypes.c_int, ctypes.c_void_p
+        _lib.oracle_xengine_ci8.argtypes = [P, L, L, L, L, L, P, I]
+        _lib.oracle_xengine_cf32.argtypes = [P, L, L, L, L, L, P, I]
+        _lib.oracle_full_matrix_ci8.argtypes = [P, L, L, L, L, P]
+        _lib.oracle_full_matrix_cf32.argtypes = [P, L, L, L, L, P]
+        _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
+        _lib.oracle_one_visibility_cf32.argtypes = [P, L, L, L, L, L, L, P]
+    return _lib
+
+
+def _check_cube(x, dtype):
+    x = np.ascontiguousarray(x)
+    if x.dtype != dtype or x.ndim != 4 or x.shape[3] != 2:
+        raise ValueError(f"expected [T][C][N][2] {dtype}, got {x.dtype} {x.shape}")
+    return x, x.shape[0], x.shape[1], x.shape[2]
+
+
+def host_threads() -> int:
+    return max(1, len(os.sched_getaffinity(0)))
+
+
+def xengine_ci8(x, c_begin=0, c_end=None, threads=1):
+    """x: int8 [T][C][N][2] -> int32 [c_end-c_begin][N(N+1)/2][2] (raw sums, i>=j row-major)."""
+    x, T, C, N = _check_cube(x, np.int8)
+    c_end = C if c_end is None else c_end
+    vis = np.empty((c_end - c_begin, N * (N + 1) // 2, 2), dtype=np.int32)
+    rc = _load().oracle_xengine_ci8(x.ctypes.data, T, C, N, c_begin, c_end, vis.ctypes.data, threads)
+    if rc == -2:
+        raise OracleOverflow("visibility does not fit int32")
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return vis
+
+
+def xengine_cf32(x, c_begin=0, c_end=None, threads=1):
+    """x: float32 [T][C][N][2] -> float64 [c_end-c_begin][N(N+1)/2][2]."""
+    x, T, C, N = _check_cube(x, np.float32)
+    c_end = C if c_end is None else c_end
+    vis = np.empty((c_end - c_begin, N * (N + 1) // 2, 2), dtype=np.float64)
+    rc = _load().oracle_xengine_cf32(x.ctypes.data, T, C, N, c_begin, c_end, vis.ctypes.data, threads)
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return vis
+
+
+def full_matrix_ci8(x, c):
+    """Full N x N matrix of channel c: int64 [N][N][2]."""
+    x, T, C, N = _check_cube(x, np.int8)
+    full = np.empty((N, N, 2), dtype=np.int64)
+    _load().oracle_full_matrix_ci8(x.ctypes.data, T, C, N, c, full.ctypes.data)
+    return full
+
+
+def full_matrix_cf32(x, c):
+    x, T, C, N = _check_cube(x, np.float32)
+    full = np.empty((N, N, 2), dtype=np.float64)
+    _load().oracle_full_matrix_cf32(x.ctypes.data, T, C, N, c, full.ctypes.data)
+    return full
+
+
+def one_visibility_ci8(x, c, i, j):
+    """(re, im) of V[c][(i,j)] as python ints."""
+    x, T, C, N = _check_cube(x, np.int8)
+    out = np.empty(2, dtype=np.int64)
+    _load().oracle_one_visibility_ci8(x.ctypes.data, T, C, N, c, i, j, out.ctypes.data)
+    return int(out[0]), int(out[1])
+
+
+def one_visibility_cf32(x, c, i, j):
+    x, T, C, N = _check_cube(x, np.float32)
+    out = np.empty(2, dtype=np.float64)
+    _load().oracle_one_visibility_cf32(x.ctypes.data, T, C, N, c, i, j, out.ctypes.data)
+    return float(out[0]), float(out[1])
