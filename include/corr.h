@@ -1,0 +1,122 @@
+/*
+ * corr.h -- C ABI of the B200 X-engine (cross-multiply-accumulate, CMAC) library.
+ *
+ * What the library computes (the operation, from the paper):
+ *   "an FX correlator ... does a channel-by-channel multiplication ('X') of the first
+ *    spectrum with the complex conjugate of the second ... accumulated for each
+ *    baseline"                                                   (sec. 2)
+ *   "The correlation products for a given frequency channel can be represented in a
+ *    matrix of size N_I x N_I formed by the outer product of a vector with its complex
+ *    conjugate"; auto-correlations on the diagonal, the two halves redundant
+ *                                                      (Fig. 2 at :115)
+ *   N_I(N_I+1)/2 products per channel, autos included
+ *   accumulators summed over the integration, then read out       (Fig. 1)
+ *
+ *   V[c][b(i,j)] = sum_{t=0}^{T-1} x[t][c][i] * conj(x[t][c][j]),  i >= j,
+ *   b(i,j) = i(i+1)/2 + j   (row-major lower triangle; readings R1, R2)
+ *
+ * Raw sums are emitted; the division by the update count the paper does at read-out
+ * is left to the caller (reading R3).
+ *
+ * Every pointer named d_* is DEVICE memory; h_* is HOST memory.  No torch types, no
+ * exceptions cross this boundary.  There is no CPU fallback: every entry point that
+ * computes needs an sm_100 device and fails with an error code otherwise.
+ */
+#ifndef CORR_H_
+#define CORR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct corr_handle corr_handle; /* opaque */
+
+/* dtype of the voltage samples */
+enum { CORR_CI8 = 0,   /* (int8 re, int8 im) -> (int32 re, int32 im), exact            */
+       CORR_CF32 = 1   /* (float re, float im) -> (float re, float im), FP32 FMA sums  */ };
+
+/* status codes */
+enum { CORR_OK = 0, CORR_EINVAL = 1, CORR_EUNSUPPORTED = 2, CORR_EALLOC = 3,
+       CORR_ECUDA = 4, CORR_EARCH = 5 };
+
+/* how the corner turn (the "unpack" transpose) is realised, CI8 only */
+enum { CORR_TURN_FUSED = 0,     /* the TMA box load of the CMAC kernel is the corner turn   */
+       CORR_TURN_STANDALONE = 1 /* corr_corner_turn into handle scratch, then the CMAC kernel */ };
+
+/*
+ * corr_create -- plan one X-engine shape on the current CUDA device.
+ *   n_inputs N_I : multiple of 32, 32..4096   (the paper needs G | N_I)
+ *   n_chan   C   : >= 1
+ *   n_time   T   : >= 1; for CORR_CI8 also T <= 65535 so that no int8 input can
+ *                  overflow int32 (|V| <= T*2*128^2; reading R6)
+ *   dtype        : CORR_CI8 or CORR_CF32
+ * Returns NULL on failure; corr_last_error()/corr_last_status() say why
+ * (CORR_EINVAL, CORR_EUNSUPPORTED shape, CORR_EARCH not sm_100, CORR_EALLOC, CORR_ECUDA).
+ * The handle owns its device workspaces (tile schedule, corner-turn scratch) until
+ * corr_destroy.  One handle is used from one host thread at a time.
+ */
+corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype);
+
+/*
+ * corr_xengine -- one whole integration.  Asynchronous on `stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream); no host sync.
+ *   d_in  : device, [n_time][n_chan][n_inputs] interleaved complex (input index fastest:
+ *           the order the paper's aggregator emits).
+ *           CI8: int8 re, int8 im (2 B/sample).  CF32: float re, float im (8 B/sample).
+ *           16-byte aligned; read only.
+ *   d_vis : device, [n_chan][N_I(N_I+1)/2] interleaved complex (int32 or float pairs),
+ *           OVERWRITTEN with the raw sums of this call (reading R4); 16-byte aligned;
+ *           must not alias d_in.  Im of every autocorrelation is exactly 0.
+ * Returns CORR_OK, CORR_EINVAL (NULL / misaligned pointers, NULL handle) or CORR_ECUDA.
+ */
+int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream);
+
+/* corr_destroy -- frees the handle's workspaces.  NULL is a no-op.  Returns CORR_OK. */
+int corr_destroy(corr_handle *h);
+
+/* Thread-local text / code of the last failure on this thread; never NULL. */
+const char *corr_last_error(void);
+int corr_last_status(void);
+
+/* Sizes in bytes of one integration's input and output for this handle. */
+size_t corr_in_bytes(const corr_handle *h);  /* T*C*N*2 (CI8) or T*C*N*8 (CF32) */
+size_t corr_vis_bytes(const corr_handle *h); /* C*N(N+1)/2*8                    */
+
+/* Number of kernel launches one corr_xengine call enqueues (for bench accounting). */
+int corr_launches_per_call(const corr_handle *h);
+
+/*
+ * corr_set_turn -- CI8 only: choose the corner-turn realisation (default CORR_TURN_FUSED).
+ * CORR_TURN_STANDALONE allocates an in_bytes-sized scratch on first use.
+ */
+int corr_set_turn(corr_handle *h, int mode);
+
+/*
+ * corr_corner_turn -- the standalone corner-turn kernel, CI8 or CF32:
+ *   d_in  [T][C][N] samples  ->  d_out [C][T][N] samples (per-channel, time-major tiles),
+ * 16-byte vectorised coalesced loads and stores through a shared-memory tile.  Pure byte
+ * permutation.  d_out has corr_in_bytes(h) bytes, 16-byte aligned, must not alias d_in.
+ */
+int corr_corner_turn(corr_handle *h, const void *d_in, void *d_out, void *stream);
+
+/*
+ * Streaming driver (staging + H2D of the next batch
+ * overlapped with the CMAC of the previous one).
+ *   h_in  : n_integrations pointers to PINNED host buffers, corr_in_bytes(h) each
+ *   d_vis : device, n_integrations * corr_vis_bytes(h) bytes (integration k at offset k*vis_bytes)
+ * Copies integration k+1 on a side stream while the X-engine runs integration k on the
+ * compute stream (two device input buffers owned by the handle).  Blocks until done.
+ * On success writes to stats (if not NULL): [0] wall seconds (host clock around the whole run),
+ * [1] device seconds (CUDA events, first copy start -> last kernel end),
+ * [2] sum of kernel seconds, [3] sum of H2D copy seconds.
+ */
+int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
+                    void *d_vis, double *stats);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CORR_H_ */

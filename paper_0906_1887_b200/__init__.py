@@ -1,0 +1,159 @@
+"""paper_0906_1887_b200 -- Python binding of the B200 X-engine C ABI (include/corr.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of libcorr.so.
+Names mirror the C entry points (corr_create / corr_xengine / corr_destroy).
+torch is used for device memory and streams, nothing else.  There is no CPU fallback: if
+libcorr.so is missing or cannot be loaded, importing the binding's functions raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+CORR_CI8, CORR_CF32 = 0, 1
+CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
+CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
+
+EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
+           "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
+           "corr_corner_turn", "corr_stream_run")
+
+_lib = None
+
+
+class CorrError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"[corr status {status}] {msg}")
+        self.status = status
+
+
+def lib():
+    """Load libcorr.so (building it in-tree first if it is stale and nvcc is present)."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if _build.stale():
+            path = _build.build()
+        L = ctypes.CDLL(path)
+        vp, ci = ctypes.c_void_p, ctypes.c_int
+        L.corr_create.restype, L.corr_create.argtypes = vp, [ci, ci, ci, ci]
+        L.corr_xengine.restype, L.corr_xengine.argtypes = ci, [vp, vp, vp, vp]
+        L.corr_destroy.restype, L.corr_destroy.argtypes = ci, [vp]
+        L.corr_last_error.restype, L.corr_last_error.argtypes = ctypes.c_char_p, []
+        L.corr_last_status.restype, L.corr_last_status.argtypes = ci, []
+        L.corr_in_bytes.restype, L.corr_in_bytes.argtypes = ctypes.c_size_t, [vp]
+        L.corr_vis_bytes.restype, L.corr_vis_bytes.argtypes = ctypes.c_size_t, [vp]
+        L.corr_launches_per_call.restype, L.corr_launches_per_call.argtypes = ci, [vp]
+        L.corr_set_turn.restype, L.corr_set_turn.argtypes = ci, [vp, ci]
+        L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
+        L.corr_stream_run.restype = ci
+        L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
+        _lib = L
+    return _lib
+
+
+def _raise():
+    L = lib()
+    raise CorrError(L.corr_last_status(), L.corr_last_error().decode())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+class Correlator:
+    """One planned X-engine shape.  Tensors are torch CUDA tensors (device memory only)."""
+
+    def __init__(self, n_inputs, n_chan, n_time, dtype):
+        self.n_inputs, self.n_chan, self.n_time = n_inputs, n_chan, n_time
+        self.dtype = {"ci8": CORR_CI8, "cf32": CORR_CF32}.get(dtype, dtype)
+        self._h = lib().corr_create(n_inputs, n_chan, n_time, self.dtype)
+        if not self._h:
+            _raise()
+        self.n_baselines = n_inputs * (n_inputs + 1) // 2
+        self.in_bytes = lib().corr_in_bytes(self._h)
+        self.vis_bytes = lib().corr_vis_bytes(self._h)
+
+    # -- corr_destroy
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().corr_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    @property
+    def launches_per_call(self):
+        return lib().corr_launches_per_call(self._h)
+
+    def set_turn(self, mode):
+        if lib().corr_set_turn(self._h, mode) != CORR_OK:
+            _raise()
+
+    def empty_vis(self, n=1):
+        import torch
+        dt = torch.int32 if self.dtype == CORR_CI8 else torch.float32
+        shape = (self.n_chan, self.n_baselines, 2) if n == 1 else (n, self.n_chan, self.n_baselines, 2)
+        return torch.empty(shape, dtype=dt, device="cuda")
+
+    def _check_in(self, d_in):
+        if not d_in.is_cuda or not d_in.is_contiguous() or d_in.numel() * d_in.element_size() != self.in_bytes:
+            raise ValueError(f"d_in must be a contiguous CUDA tensor of {self.in_bytes} bytes "
+                             f"([T][C][N][2] int8 or float32)")
+
+    # -- corr_xengine
+    def xengine(self, d_in, d_vis=None, stream=None):
+        """d_in: CUDA [T][C][N][2] int8|float32 -> d_vis: CUDA [C][N(N+1)/2][2] int32|float32 (raw sums)."""
+        self._check_in(d_in)
+        if d_vis is None:
+            d_vis = self.empty_vis()
+        if not d_vis.is_cuda or not d_vis.is_contiguous() or d_vis.numel() * d_vis.element_size() != self.vis_bytes:
+            raise ValueError(f"d_vis must be a contiguous CUDA tensor of {self.vis_bytes} bytes")
+        rc = lib().corr_xengine(self._h, d_in.data_ptr(), d_vis.data_ptr(), _stream_ptr(stream))
+        if rc != CORR_OK:
+            _raise()
+        return d_vis
+
+    # -- corr_corner_turn
+    def corner_turn(self, d_in, d_out=None, stream=None):
+        import torch
+        self._check_in(d_in)
+        if d_out is None:
+            d_out = torch.empty_like(d_in)
+        rc = lib().corr_corner_turn(self._h, d_in.data_ptr(), d_out.data_ptr(), _stream_ptr(stream))
+        if rc != CORR_OK:
+            _raise()
+        return d_out
+
+    # -- corr_stream_run
+    def stream_run(self, h_in_list, d_vis=None):
+        """h_in_list: pinned host tensors, one per integration.  Returns (d_vis, stats dict)."""
+        n = len(h_in_list)
+        for t in h_in_list:
+            if t.is_cuda or not t.is_pinned() or t.numel() * t.element_size() != self.in_bytes:
+                raise ValueError("stream_run needs pinned host tensors of in_bytes each")
+        if d_vis is None:
+            d_vis = self.empty_vis(n)
+        ptrs = (ctypes.c_void_p * n)(*[t.data_ptr() for t in h_in_list])
+        stats = (ctypes.c_double * 4)()
+        rc = lib().corr_stream_run(self._h, ptrs, n, d_vis.data_ptr(), stats)
+        if rc != CORR_OK:
+            _raise()
+        return d_vis, {"wall_s": stats[0], "device_s": stats[1], "kernel_s": stats[2], "h2d_s": stats[3]}
+
+
+def corr_create(n_inputs, n_chan, n_time, dtype):
+    return Correlator(n_inputs, n_chan, n_time, dtype)
+
+
+def corr_xengine(handle, d_in, d_vis=None, stream=None):
+    return handle.xengine(d_in, d_vis, stream)
+
+
+def corr_destroy(handle):
+    handle.destroy()

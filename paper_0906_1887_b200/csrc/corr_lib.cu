@@ -1,0 +1,437 @@
+// corr_lib.cu -- host side of the C ABI declared in include/corr.h.
+// Plans the tile schedule (descendant of the paper's constant-memory pair lookup table,
+// PAPER.md:117), encodes TMA tensor maps, launches the sm_100a kernels.  No CPU compute path.
+#include "../../include/corr.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <queue>
+#include <vector>
+
+#include "corner_turn.cuh"
+#include "xengine_f32.cuh"
+#include "xengine_i8.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+thread_local int g_status = CORR_OK;
+
+int fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  g_status = code;
+  return code;
+}
+#define CUDA_TRY(call)                                                                        \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) return fail(CORR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+struct MapCacheEntry {
+  const void *ptr;
+  CUtensorMap map;
+};
+
+}  // namespace
+
+struct corr_handle {
+  int n_inputs, n_chan, n_time, dtype;
+  long long n_baselines;
+  size_t in_bytes, vis_bytes;
+  int n_sms;
+  int turn_mode;
+  // CI8 plan
+  int pair_mode, panels, bk, slots, stages, grid_i8;
+  size_t smem_i8;
+  int4 *d_items_i8;
+  int *d_offsets_i8;
+  int n_items_i8;
+  void *d_scratch;  // corner-turn output (standalone mode)
+  std::vector<MapCacheEntry> maps;
+  // CF32 plan
+  int2 *d_items_f32;
+  int n_items_f32;
+  int f32_threads;
+  // streaming driver
+  void *d_stream_in[2];
+  cudaStream_t s_copy, s_compute;
+};
+
+namespace {
+
+// Static balanced schedule: items in channel-major order (so that CTAs running at the same time
+// share a channel's panels in L2), each given to the least-loaded CTA so far.
+void plan_i8(corr_handle *h, std::vector<int4> &items, std::vector<int> &offsets) {
+  const int N = h->n_inputs;
+  h->pair_mode = (N == 32) ? 1 : 0;
+  h->panels = h->pair_mode ? 1 : (2 * N + 127) / 128;
+  const int groups = h->pair_mode ? (h->n_chan + 1) / 2 : h->n_chan;
+  h->slots = h->panels <= 4 ? h->panels : 5;
+  h->bk = h->slots == 1 ? 256 : h->slots == 2 ? 128 : 64;
+  const size_t stage_bytes = static_cast<size_t>(h->slots) * h->bk * 128;
+  h->stages = static_cast<int>(std::min<size_t>(corr::kMaxStages, (220 * 1024) / stage_bytes));
+  h->smem_i8 = stage_bytes * h->stages + 1024;
+
+  struct Raw { int4 it; long long cost; };
+  std::vector<Raw> raw;
+  for (int g = 0; g < groups; ++g) {
+    const int chan = h->pair_mode ? 2 * g : g;
+    for (int I = h->panels - 1; I >= 0; --I)
+      for (int J0 = 0; J0 <= I; J0 += 4) {
+        const int nJ = std::min(4, I - J0 + 1);
+        const bool a_in_b = I < J0 + nJ;
+        const long long cost = 2LL * h->n_time * nJ + 700LL * nJ + 64LL * h->n_time / 32 * (a_in_b ? 0 : 0) + 1500;
+        raw.push_back({make_int4(chan, I | (J0 << 16), nJ, 0), cost});
+      }
+  }
+  h->n_items_i8 = static_cast<int>(raw.size());
+  h->grid_i8 = std::min(h->n_items_i8, h->n_sms);
+  std::vector<std::vector<int4>> per(h->grid_i8);
+  typedef std::pair<long long, int> LB;  // (load, cta)
+  std::priority_queue<LB, std::vector<LB>, std::greater<LB>> pq;
+  for (int b = 0; b < h->grid_i8; ++b) pq.push({0, b});
+  for (const Raw &r : raw) {
+    LB lb = pq.top();
+    pq.pop();
+    per[lb.second].push_back(r.it);
+    pq.push({lb.first + r.cost, lb.second});
+  }
+  offsets.assign(1, 0);
+  for (int b = 0; b < h->grid_i8; ++b) {
+    items.insert(items.end(), per[b].begin(), per[b].end());
+    offsets.push_back(static_cast<int>(items.size()));
+  }
+}
+
+void plan_f32(corr_handle *h, std::vector<int2> &items) {
+  const int blocks = (h->n_inputs + corr::kF32Block - 1) / corr::kF32Block;
+  for (int c = 0; c < h->n_chan; ++c)
+    for (int I = 0; I < blocks; ++I)
+      for (int J = 0; J <= I; ++J) items.push_back(make_int2(c, I | (J << 16)));
+  h->n_items_f32 = static_cast<int>(items.size());
+  h->f32_threads = blocks == 1 ? 160 : corr::kF32Threads;  // 136 active tiles on a diagonal block
+}
+
+int encode_map(corr_handle *h, const void *base, bool turned, CUtensorMap *out) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return fail(CORR_ECUDA, "cuTensorMapEncodeTiled entry point not available");
+  const cuuint64_t row = static_cast<cuuint64_t>(2) * h->n_inputs;  // bytes per (t, c)
+  CUresult r;
+  if (!turned) {
+    cuuint64_t dims[2] = {row * h->n_chan, static_cast<cuuint64_t>(h->n_time)};
+    cuuint64_t strides[1] = {row * h->n_chan};
+    cuuint32_t box[2] = {128, static_cast<cuuint32_t>(h->bk)};
+    cuuint32_t es[2] = {1, 1};
+    r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  } else {
+    const cuuint64_t grow = h->pair_mode ? 2 * row : row;
+    const cuuint64_t groups = h->pair_mode ? h->n_chan / 2 : h->n_chan;
+    cuuint64_t dims[3] = {grow, static_cast<cuuint64_t>(h->n_time), groups};
+    cuuint64_t strides[2] = {grow, grow * h->n_time};
+    cuuint32_t box[3] = {128, static_cast<cuuint32_t>(h->bk), 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
+  if (r != CUDA_SUCCESS) return fail(CORR_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return CORR_OK;
+}
+
+int get_map(corr_handle *h, const void *base, bool turned, const CUtensorMap **out) {
+  for (const MapCacheEntry &e : h->maps)
+    if (e.ptr == base) { *out = &e.map; return CORR_OK; }
+  if (h->maps.size() >= 64) h->maps.erase(h->maps.begin());
+  MapCacheEntry e;
+  e.ptr = base;
+  int rc = encode_map(h, base, turned, &e.map);
+  if (rc != CORR_OK) return rc;
+  h->maps.push_back(e);
+  *out = &h->maps.back().map;
+  return CORR_OK;
+}
+
+}  // namespace
+
+// ============================================================================ C ABI
+extern "C" {
+
+const char *corr_last_error(void) { return g_err; }
+int corr_last_status(void) { return g_status; }
+
+corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
+  g_status = CORR_OK;
+  g_err[0] = 0;
+  if (n_inputs <= 0 || n_chan <= 0 || n_time <= 0) {
+    fail(CORR_EINVAL, "corr_create: n_inputs, n_chan, n_time must be positive (got %d, %d, %d)", n_inputs, n_chan, n_time);
+    return nullptr;
+  }
+  if (dtype != CORR_CI8 && dtype != CORR_CF32) {
+    fail(CORR_EINVAL, "corr_create: unknown dtype %d", dtype);
+    return nullptr;
+  }
+  if (n_inputs % 32 != 0 || n_inputs > 4096) {
+    fail(CORR_EUNSUPPORTED, "corr_create: n_inputs must be a multiple of 32 and <= 4096 (got %d)", n_inputs);
+    return nullptr;
+  }
+  if (dtype == CORR_CI8 && n_time > 65535) {
+    fail(CORR_EUNSUPPORTED, "corr_create: CI8 needs n_time <= 65535 so that int32 cannot overflow (got %d)", n_time);
+    return nullptr;
+  }
+  if (static_cast<unsigned long long>(n_chan) * n_inputs * 2ull >= (1ull << 31)) {
+    fail(CORR_EUNSUPPORTED, "corr_create: n_chan * n_inputs too large");
+    return nullptr;
+  }
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    fail(CORR_ECUDA, "corr_create: no usable CUDA device (%s)", cudaGetErrorString(cudaGetLastError()));
+    return nullptr;
+  }
+  if (prop.major != 10) {
+    fail(CORR_EARCH, "corr_create: device is sm_%d%d; this library is sm_100a only", prop.major, prop.minor);
+    return nullptr;
+  }
+  corr_handle *h = new (std::nothrow) corr_handle();
+  if (!h) {
+    fail(CORR_EALLOC, "corr_create: host allocation failed");
+    return nullptr;
+  }
+  h->n_inputs = n_inputs;
+  h->n_chan = n_chan;
+  h->n_time = n_time;
+  h->dtype = dtype;
+  h->n_baselines = static_cast<long long>(n_inputs) * (n_inputs + 1) / 2;
+  h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * (dtype == CORR_CI8 ? 2 : 8);
+  h->vis_bytes = static_cast<size_t>(n_chan) * h->n_baselines * 8;
+  h->n_sms = prop.multiProcessorCount;
+  h->turn_mode = CORR_TURN_FUSED;
+  h->d_items_i8 = nullptr;
+  h->d_offsets_i8 = nullptr;
+  h->d_items_f32 = nullptr;
+  h->d_scratch = nullptr;
+  h->d_stream_in[0] = h->d_stream_in[1] = nullptr;
+  h->s_copy = h->s_compute = nullptr;
+
+  cudaError_t e = cudaSuccess;
+  if (dtype == CORR_CI8) {
+    std::vector<int4> items;
+    std::vector<int> offsets;
+    plan_i8(h, items, offsets);
+    e = cudaMalloc(&h->d_items_i8, items.size() * sizeof(int4));
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_offsets_i8, offsets.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_items_i8, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_offsets_i8, offsets.data(), offsets.size() * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
+  } else {
+    std::vector<int2> items;
+    plan_f32(h, items);
+    e = cudaMalloc(&h->d_items_f32, items.size() * sizeof(int2));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_items_f32, items.data(), items.size() * sizeof(int2), cudaMemcpyHostToDevice);
+  }
+  if (e != cudaSuccess) {
+    fail(e == cudaErrorMemoryAllocation ? CORR_EALLOC : CORR_ECUDA, "corr_create: %s", cudaGetErrorString(e));
+    corr_destroy(h);
+    return nullptr;
+  }
+  return h;
+}
+
+int corr_destroy(corr_handle *h) {
+  if (!h) return CORR_OK;
+  cudaFree(h->d_items_i8);
+  cudaFree(h->d_offsets_i8);
+  cudaFree(h->d_items_f32);
+  cudaFree(h->d_scratch);
+  cudaFree(h->d_stream_in[0]);
+  cudaFree(h->d_stream_in[1]);
+  if (h->s_copy) cudaStreamDestroy(h->s_copy);
+  if (h->s_compute) cudaStreamDestroy(h->s_compute);
+  delete h;
+  return CORR_OK;
+}
+
+size_t corr_in_bytes(const corr_handle *h) { return h ? h->in_bytes : 0; }
+size_t corr_vis_bytes(const corr_handle *h) { return h ? h->vis_bytes : 0; }
+int corr_launches_per_call(const corr_handle *h) {
+  if (!h) return 0;
+  return (h->dtype == CORR_CI8 && h->turn_mode == CORR_TURN_STANDALONE) ? 2 : 1;
+}
+
+int corr_set_turn(corr_handle *h, int mode) {
+  if (!h) return fail(CORR_EINVAL, "corr_set_turn: NULL handle");
+  if (h->dtype != CORR_CI8) return fail(CORR_EUNSUPPORTED, "corr_set_turn: only the CI8 path has two corner-turn realisations");
+  if (mode != CORR_TURN_FUSED && mode != CORR_TURN_STANDALONE) return fail(CORR_EINVAL, "corr_set_turn: unknown mode %d", mode);
+  if (mode == CORR_TURN_STANDALONE) {
+    if (h->pair_mode && (h->n_chan & 1))
+      return fail(CORR_EUNSUPPORTED, "corr_set_turn: standalone turn with n_inputs == 32 needs an even n_chan");
+    if (!h->d_scratch) {
+      cudaError_t e = cudaMalloc(&h->d_scratch, h->in_bytes);
+      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_set_turn: scratch of %zu bytes: %s", h->in_bytes, cudaGetErrorString(e));
+    }
+  }
+  h->turn_mode = mode;
+  return CORR_OK;
+}
+
+static int launch_turn(corr_handle *h, const void *d_in, void *d_out, cudaStream_t st) {
+  corr::TurnParams tp;
+  const size_t w = static_cast<size_t>(h->n_inputs) * (h->dtype == CORR_CI8 ? 2 : 8);
+  const bool pair = (h->dtype == CORR_CI8) && h->pair_mode;
+  const size_t wg = pair ? 2 * w : w;
+  tp.in = static_cast<const uint4 *>(d_in);
+  tp.out = static_cast<uint4 *>(d_out);
+  tp.n_time = h->n_time;
+  tp.n_groups = pair ? h->n_chan / 2 : h->n_chan;
+  tp.wc = static_cast<int>(wg / 16);
+  const int max_rows = static_cast<int>(corr::kTurnTileBytes / wg);  // (t, g) rows per tile
+  if (max_rows < 1) return fail(CORR_EUNSUPPORTED, "corr_corner_turn: row of %zu bytes exceeds the tile", wg);
+  tp.tt = std::min(std::min(32, max_rows), h->n_time);
+  tp.gg = std::max(1, std::min(max_rows / tp.tt, tp.n_groups));
+  dim3 grid((tp.n_groups + tp.gg - 1) / tp.gg, (tp.n_time + tp.tt - 1) / tp.tt);
+  corr::corner_turn_kernel<<<grid, corr::kTurnThreads, 0, st>>>(tp);
+  CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
+int corr_corner_turn(corr_handle *h, const void *d_in, void *d_out, void *stream) {
+  if (!h || !d_in || !d_out) return fail(CORR_EINVAL, "corr_corner_turn: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_out)) & 15)
+    return fail(CORR_EINVAL, "corr_corner_turn: pointers must be 16-byte aligned");
+  if (d_in == d_out) return fail(CORR_EINVAL, "corr_corner_turn: d_in and d_out alias");
+  if (h->dtype == CORR_CI8 && h->pair_mode && (h->n_chan & 1))
+    return fail(CORR_EUNSUPPORTED, "corr_corner_turn: n_inputs == 32 needs an even n_chan");
+  return launch_turn(h, d_in, d_out, static_cast<cudaStream_t>(stream));
+}
+
+int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
+  if (!h) return fail(CORR_EINVAL, "corr_xengine: NULL handle");
+  if (!d_in || !d_vis) return fail(CORR_EINVAL, "corr_xengine: NULL device pointer");
+  if ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_vis)) & 15)
+    return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis must be 16-byte aligned");
+  if (d_in == d_vis) return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis alias");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (h->dtype == CORR_CF32) {
+    corr::F32Params fp;
+    fp.in = static_cast<const float2 *>(d_in);
+    fp.vis = static_cast<float2 *>(d_vis);
+    fp.items = h->d_items_f32;
+    fp.n_items = h->n_items_f32;
+    fp.n_time = h->n_time;
+    fp.n_chan = h->n_chan;
+    fp.n_inputs = h->n_inputs;
+    fp.n_baselines = h->n_baselines;
+    corr::xengine_f32_kernel<<<h->n_items_f32, h->f32_threads, 0, st>>>(fp);
+    CUDA_TRY(cudaGetLastError());
+    return CORR_OK;
+  }
+  const bool turned = h->turn_mode == CORR_TURN_STANDALONE;
+  const void *src = d_in;
+  if (turned) {
+    int rc = launch_turn(h, d_in, h->d_scratch, st);
+    if (rc != CORR_OK) return rc;
+    src = h->d_scratch;
+  }
+  const CUtensorMap *map = nullptr;
+  int rc = get_map(h, src, turned, &map);
+  if (rc != CORR_OK) return rc;
+  corr::I8Params ip;
+  ip.items = h->d_items_i8;
+  ip.offsets = h->d_offsets_i8;
+  ip.n_time = h->n_time;
+  ip.n_inputs = h->n_inputs;
+  ip.n_chan = h->n_chan;
+  ip.pair_mode = h->pair_mode;
+  ip.bk = h->bk;
+  ip.slots = h->slots;
+  ip.stages = h->stages;
+  ip.turned = turned ? 1 : 0;
+  ip.n_baselines = h->n_baselines;
+  ip.vis = static_cast<int2 *>(d_vis);
+  corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(*map, ip);
+  CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
+int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations, void *d_vis, double *stats) {
+  if (!h || !h_in || !d_vis || n_integrations <= 0) return fail(CORR_EINVAL, "corr_stream_run: bad argument");
+  for (int k = 0; k < n_integrations; ++k)
+    if (!h_in[k]) return fail(CORR_EINVAL, "corr_stream_run: h_in[%d] is NULL", k);
+  if (!h->s_copy) CUDA_TRY(cudaStreamCreateWithFlags(&h->s_copy, cudaStreamNonBlocking));
+  if (!h->s_compute) CUDA_TRY(cudaStreamCreateWithFlags(&h->s_compute, cudaStreamNonBlocking));
+  for (int b = 0; b < 2; ++b)
+    if (!h->d_stream_in[b]) {
+      cudaError_t e = cudaMalloc(&h->d_stream_in[b], h->in_bytes);
+      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_stream_run: input buffer of %zu bytes: %s", h->in_bytes, cudaGetErrorString(e));
+    }
+  const int n = n_integrations;
+  std::vector<cudaEvent_t> ev(4 * n);  // per integration: copy start, copy end, kernel start, kernel end
+  for (cudaEvent_t &e : ev) CUDA_TRY(cudaEventCreate(&e));
+  int rc = CORR_OK;
+  const auto w0 = std::chrono::steady_clock::now();
+  for (int k = 0; k < n && rc == CORR_OK; ++k) {
+    const int b = k & 1;
+    // buffer b is free once the kernel of integration k-2 has finished reading it
+    if (k >= 2) cudaStreamWaitEvent(h->s_copy, ev[4 * (k - 2) + 3], 0);
+    cudaEventRecord(ev[4 * k + 0], h->s_copy);
+    cudaMemcpyAsync(h->d_stream_in[b], h_in[k], h->in_bytes, cudaMemcpyHostToDevice, h->s_copy);
+    cudaEventRecord(ev[4 * k + 1], h->s_copy);
+    cudaStreamWaitEvent(h->s_compute, ev[4 * k + 1], 0);
+    cudaEventRecord(ev[4 * k + 2], h->s_compute);
+    rc = corr_xengine(h, h->d_stream_in[b], static_cast<char *>(d_vis) + static_cast<size_t>(k) * h->vis_bytes, h->s_compute);
+    cudaEventRecord(ev[4 * k + 3], h->s_compute);
+  }
+  cudaError_t e1 = cudaStreamSynchronize(h->s_copy);
+  cudaError_t e2 = cudaStreamSynchronize(h->s_compute);
+  const auto w1 = std::chrono::steady_clock::now();
+  if (rc == CORR_OK && (e1 != cudaSuccess || e2 != cudaSuccess))
+    rc = fail(CORR_ECUDA, "corr_stream_run: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+  if (rc == CORR_OK && stats) {
+    float ms = 0.f;
+    double ksum = 0.0, csum = 0.0;
+    cudaEventElapsedTime(&ms, ev[0], ev[4 * (n - 1) + 3]);
+    stats[0] = std::chrono::duration<double>(w1 - w0).count();
+    stats[1] = ms * 1e-3;
+    for (int k = 0; k < n; ++k) {
+      cudaEventElapsedTime(&ms, ev[4 * k + 2], ev[4 * k + 3]);
+      ksum += ms * 1e-3;
+      cudaEventElapsedTime(&ms, ev[4 * k + 0], ev[4 * k + 1]);
+      csum += ms * 1e-3;
+    }
+    stats[2] = ksum;
+    stats[3] = csum;
+  }
+  for (cudaEvent_t &e : ev) cudaEventDestroy(e);
+  return rc;
+}
+
+}  // extern "C"

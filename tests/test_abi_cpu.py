@@ -1,0 +1,92 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol that
+include/corr.h declares; the product never reaches into oracle/ (and vice versa); without a GPU
+the compute entry points fail loudly instead of falling back."""
+from __future__ import annotations
+
+import ast
+import os
+import re
+import shutil
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+needs_nvcc = pytest.mark.skipif(shutil.which("nvcc") is None and not os.path.exists(
+    os.path.join(ROOT, "paper_0906_1887_b200", "libcorr.so")), reason="no nvcc and no prebuilt libcorr.so")
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "corr.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(corr_[a-z0-9_]+)\s*\(", text)))
+
+
+@needs_nvcc
+def test_library_exports_every_declared_symbol():
+    import paper_0906_1887_b200 as pkg
+    L = pkg.lib()
+    syms = header_symbols()
+    assert {"corr_create", "corr_xengine", "corr_destroy"} <= set(syms)
+    for s in syms:
+        assert hasattr(L, s), f"{s} declared in include/corr.h but not exported"
+    assert set(pkg.EXPORTS) == set(syms)
+
+
+@needs_nvcc
+def test_no_cpu_fallback_without_device():
+    torch = pytest.importorskip("torch")
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    import paper_0906_1887_b200 as pkg
+    with pytest.raises(pkg.CorrError) as e:
+        pkg.corr_create(64, 2, 10, "ci8")
+    assert e.value.status in (pkg.CORR_ECUDA, pkg.CORR_EARCH)
+    # argument validation happens before any device work and needs no GPU
+    for bad in [(48, 2, 10, "ci8"), (64, 2, 70000, "ci8"), (64, 0, 10, "cf32")]:
+        with pytest.raises(pkg.CorrError) as e:
+            pkg.corr_create(*bad)
+        assert e.value.status in (pkg.CORR_EINVAL, pkg.CORR_EUNSUPPORTED)
+    L = pkg.lib()
+    assert L.corr_destroy(None) == pkg.CORR_OK
+    assert L.corr_xengine(None, None, None, None) == pkg.CORR_EINVAL
+
+
+def _imports(path):
+    tree = ast.parse(open(path).read())
+    names = set()
+    for node in ast.walk(tree):
+        if isinstance(node, ast.Import):
+            names |= {a.name.split(".")[0] for a in node.names}
+        elif isinstance(node, ast.ImportFrom) and node.module and node.level == 0:
+            names.add(node.module.split(".")[0])
+    return names
+
+
+def test_product_and_oracle_are_independent():
+    pkg_dir = os.path.join(ROOT, "paper_0906_1887_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            p = os.path.join(dirpath, f)
+            if f.endswith(".py"):
+                assert "oracle" not in _imports(p), f"{p} imports the oracle"
+            if f.endswith((".cu", ".cuh", ".h", ".py")):
+                assert "oracle/" not in open(p).read().replace("oracle/.", ""), f"{p} references oracle/"
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        p = os.path.join(ROOT, "oracle", f)
+        if f.endswith(".py"):
+            assert "paper_0906_1887_b200" not in _imports(p)
+        if f.endswith((".c", ".h")):
+            src = open(p).read()
+            assert "#include \"../" not in src and "csrc" not in src
+    # the generators hold none of the method's arithmetic and import neither side
+    gen = _imports(os.path.join(ROOT, "corrgen", "__init__.py"))
+    assert "oracle" not in gen and "paper_0906_1887_b200" not in gen
+    # bench.py may use the oracle only in its cpu_baseline / reference legs
+    bench = os.path.join(ROOT, "bench.py")
+    if os.path.exists(bench):
+        src = open(bench).read()
+        for m in re.finditer(r"^\s*import oracle|^\s*from oracle", src, flags=re.M):
+            pre = src[:m.start()]
+            fn = re.findall(r"^def (\w+)", pre, flags=re.M)[-1]
+            assert fn in ("cpu_baseline", "run_reference"), f"bench.py imports oracle inside {fn}()"

@@ -1,0 +1,192 @@
+"""GPU parity: the CUDA X-engine (through the C ABI binding) vs the CPU oracle, element by element.
+
+int8 path: bit-exact.  float32 path: |delta| <= 1e-5 sqrt(|V_ii V_jj|) against the float64 oracle
+(north_star).  Inputs are the seeded synthetic recipes of DESIGN.md.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import corrgen
+import oracle
+from parity_util import f32_tolerance_check
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import paper_0906_1887_b200 as p
+    p.lib()
+    return p
+
+
+def _threads():
+    return oracle.host_threads()
+
+
+def run_ci8(pkg, x, turn=None):
+    T, C, N, _ = x.shape
+    h = pkg.corr_create(N, C, T, "ci8")
+    if turn is not None:
+        h.set_turn(turn)
+    d_in = torch.from_numpy(x).cuda()
+    vis = h.empty_vis()
+    vis.fill_(-0x55555555)  # poison: every element must be overwritten
+    pkg.corr_xengine(h, d_in, vis)
+    torch.cuda.synchronize()
+    out = vis.cpu().numpy()
+    pkg.corr_destroy(h)
+    return out
+
+
+def run_cf32(pkg, x):
+    T, C, N, _ = x.shape
+    h = pkg.corr_create(N, C, T, "cf32")
+    d_in = torch.from_numpy(x).cuda()
+    vis = h.empty_vis()
+    vis.fill_(float("nan"))
+    pkg.corr_xengine(h, d_in, vis)
+    torch.cuda.synchronize()
+    out = vis.cpu().numpy()
+    pkg.corr_destroy(h)
+    return out
+
+
+# (N, C, T): several tiles + ragged tails; T in {1,31,32,33} pins K zero-padding (reading R11);
+# N=32 exercises the two-channels-per-panel mode incl. odd C; N=96/320/640 multi-panel, separate-A
+# and multi-segment items; N=1024 the c4 tile schedule.
+CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (64, 1, 257), (64, 200, 40),
+              (32, 4, 100), (32, 3, 70), (32, 1, 64), (32, 301, 33), (96, 2, 64), (128, 2, 300),
+              (256, 2, 130), (320, 1, 64), (640, 1, 40), (1024, 1, 96)]
+
+
+@pytest.mark.parametrize("N,C,T", CI8_SHAPES)
+def test_ci8_gauss_bit_exact(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("N,C,T", [(64, 3, 100), (256, 2, 130), (32, 4, 100)])
+def test_ci8_uniform_full_range_bit_exact(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c3"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+
+
+def test_ci8_zero_input(pkg):
+    x = np.zeros((40, 3, 64, 2), np.int8)
+    assert not run_ci8(pkg, x).any()
+
+
+@pytest.mark.parametrize("val", [-128, 127])
+def test_ci8_extreme_constant_longest_integration(pkg, val):
+    """T = 65535 with every component at +-full scale: the largest sums the ABI admits (reading R6)."""
+    x = np.full((65535, 2, 32, 2), val, np.int8)
+    out = run_ci8(pkg, x)
+    assert np.array_equal(out, oracle.xengine_ci8(x, threads=_threads()))
+    assert out[..., 0].max() == 65535 * 2 * val * val
+
+
+@pytest.mark.parametrize("N,C,T", [(64, 6, 100), (32, 4, 70), (256, 2, 64), (96, 2, 40)])
+def test_ci8_standalone_corner_turn_path(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x, turn=pkg.CORR_TURN_STANDALONE), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("dtype,N,C,T", [("ci8", 64, 7, 100), ("ci8", 32, 6, 33), ("ci8", 1024, 3, 20),
+                                         ("cf32", 64, 5, 50), ("cf32", 32, 3, 17)])
+def test_corner_turn_is_the_permutation(pkg, dtype, N, C, T):
+    """[T][C][N] -> [C][T][N] (channel pairs for N_I = 32 int8): pure byte permutation, bit-exact."""
+    rng = np.random.default_rng(5)
+    if dtype == "ci8":
+        x = rng.integers(-128, 128, size=(T, C, N, 2), dtype=np.int8)
+    else:
+        x = rng.standard_normal((T, C, N, 2)).astype(np.float32)
+    h = pkg.corr_create(N, C, T, dtype)
+    out = h.corner_turn(torch.from_numpy(x).cuda()).cpu().numpy()
+    pkg.corr_destroy(h)
+    if dtype == "ci8" and N == 32:
+        want = x.reshape(T, C // 2, 2 * N, 2).transpose(1, 0, 2, 3)
+    else:
+        want = x.transpose(1, 0, 2, 3)
+    assert np.array_equal(out.reshape(want.shape), want)
+
+
+CF32_SHAPES = [(64, 3, 50), (64, 2, 500), (64, 40, 17), (32, 3, 33), (96, 2, 20), (128, 2, 40), (192, 1, 30)]
+
+
+@pytest.mark.parametrize("N,C,T", CF32_SHAPES)
+def test_cf32_within_tolerance(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c5"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    f32_tolerance_check(run_cf32(pkg, x), oracle.xengine_cf32(x, threads=_threads()), N)
+
+
+def test_cf32_single_nonzero_input_exact_zeros(pkg):
+    """Only input k non-zero: every other visibility is exactly 0 (oracle pin P3 on the GPU)."""
+    x = np.zeros((30, 2, 64, 2), np.float32)
+    x[:, :, 9, :] = np.random.default_rng(1).standard_normal((30, 2, 2)).astype(np.float32)
+    out = run_cf32(pkg, x)
+    ref = oracle.xengine_cf32(x)
+    f32_tolerance_check(out, ref, 64)
+    b = 9 * 10 // 2 + 9
+    mask = np.ones(out.shape[1], bool)
+    mask[b] = False
+    assert not out[:, mask].any()
+
+
+def test_overwrite_semantics_and_reuse(pkg):
+    """d_vis is overwritten each call (reading R4); one handle serves several inputs and streams."""
+    w = corrgen.scaled(corrgen.CONFIGS["c1"], n_chan=6, n_time=90)
+    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, "ci8")
+    vis = h.empty_vis()
+    s = torch.cuda.Stream()
+    for k in range(3):
+        x = w.generate(integration=k)
+        d_in = torch.from_numpy(x).cuda()
+        torch.cuda.synchronize()
+        pkg.corr_xengine(h, d_in, vis, stream=s)
+        s.synchronize()
+        assert np.array_equal(vis.cpu().numpy(), oracle.xengine_ci8(x))
+    pkg.corr_destroy(h)
+
+
+def test_stream_run_matches_oracle(pkg):
+    """Streaming driver: 5 integrations through pinned host buffers, cf32 and ci8."""
+    for dtype, key in (("cf32", "c5"), ("ci8", "c2")):
+        w = corrgen.scaled(corrgen.CONFIGS[key], n_chan=8, n_time=60)
+        xs = [w.generate(integration=k) for k in range(5)]
+        h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, dtype)
+        pinned = [torch.from_numpy(x).pin_memory() for x in xs]
+        d_vis, stats = h.stream_run(pinned)
+        out = d_vis.cpu().numpy()
+        pkg.corr_destroy(h)
+        assert stats["device_s"] > 0 and stats["kernel_s"] > 0
+        for k, x in enumerate(xs):
+            if dtype == "ci8":
+                assert np.array_equal(out[k], oracle.xengine_ci8(x))
+            else:
+                f32_tolerance_check(out[k], oracle.xengine_cf32(x), w.n_inputs)
+
+
+def test_abi_errors_on_device(pkg):
+    L = pkg.lib()
+    h = pkg.corr_create(64, 2, 10, "ci8")
+    good = torch.zeros(h.in_bytes + 64, dtype=torch.int8, device="cuda")
+    vis = h.empty_vis()
+    assert L.corr_xengine(h._h, None, vis.data_ptr(), None) == pkg.CORR_EINVAL
+    assert L.corr_xengine(h._h, good.data_ptr() + 1, vis.data_ptr(), None) == pkg.CORR_EINVAL
+    assert L.corr_xengine(None, good.data_ptr(), vis.data_ptr(), None) == pkg.CORR_EINVAL
+    assert L.corr_xengine(h._h, good.data_ptr(), good.data_ptr(), None) == pkg.CORR_EINVAL
+    assert b"corr_xengine" in L.corr_last_error()
+    pkg.corr_destroy(h)
+    for bad in [(48, 2, 10, "ci8"), (64, 2, 70000, "ci8"), (0, 1, 1, "ci8"), (64, 1, 1, 7)]:
+        with pytest.raises(pkg.CorrError):
+            pkg.corr_create(*bad)
+    assert L.corr_destroy(None) == pkg.CORR_OK
