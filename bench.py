@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- X-engine throughput on B200 (complex MACs/s) and fraction of the relevant roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--no-sweep] [--impl reference]
+
+One "step" = one corr_xengine call (the whole hot path: fused corner turn, CMAC, epilogue) over one
+integration of the named config's seeded synthetic input.  The headline
+workload is BASELINE.json configs[1] (c2: N_I=64, 768 channels, T=10000; 6x the paper's one-second
+workload).  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "xengine_complex_macs_per_s"
+UNIT = "CMAC/s"
+L2_BYTES = 126 * 1024 * 1024
+# provisional arithmetic peaks: int8 dense = 2 x measured bf16 burst; FP32 FMA = 148 SM x 128 x 2 x f
+FP32_PEAK_FLOPS = 148 * 128 * 2 * 1.965e9
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback"}
+
+
+def roofline_times(w, peaks):
+    """(t_hbm, t_alu) seconds per integration: north_star's lower-of-two roofline."""
+    t_a = w.in_bytes / (peaks["hbm_gbs"] * 1e9)
+    ops = 8.0 * w.cmacs
+    peak_ops = 2.0 * peaks["bf16_tflops"] * 1e12 if w.dtype == "ci8" else FP32_PEAK_FLOPS
+    return t_a, ops / peak_ops
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index=0, period=0.01):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.stop_flag = period, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {getattr(nv, k): k for k in dir(nv) if k.startswith("nvmlClocksEventReason") or
+                 k.startswith("nvmlClocksThrottleReason")}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                for bit, name in names.items():
+                    if isinstance(bit, int) and bit and (r & bit) and bit & (bit - 1) == 0:
+                        self.reasons.add(name.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", ""))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        s = sorted(self.samples)
+        busy = [x for x in s if self.max_mhz is None or x > 0.3 * self.max_mhz] or s
+        return {"sm_mhz": busy[len(busy) // 2] if busy else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(r for r in self.reasons if r not in ("GpuIdle", "None", "All"))}
+
+
+def make_inputs(w, n_buffers, torch, rank=0):
+    """n_buffers distinct device-resident integrations (rotated when one buffer fits in L2)."""
+    return [torch.from_numpy(w.generate(integration=k + 1000 * rank)).cuda() for k in range(n_buffers)]
+
+
+def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None):
+    """Device-resident timing of `steps` corr_xengine calls.  Returns dict with per-step seconds."""
+    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, w.dtype)
+    n_buf = 1 if w.in_bytes > 2 * L2_BYTES else min(64, -(-3 * L2_BYTES // w.in_bytes))
+    bufs = make_inputs(w, n_buf, torch, rank)
+    vis = h.empty_vis()
+    stream = torch.cuda.current_stream()
+    for k in range(warmup):
+        h.xengine(bufs[k % n_buf], vis, stream)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    ev[0].record(stream)
+    for k in range(steps):
+        h.xengine(bufs[k % n_buf], vis, stream)
+        ev[k + 1].record(stream)
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.stop_flag = True
+    total = ev[0].elapsed_time(ev[steps]) * 1e-3
+    per = sorted(ev[k].elapsed_time(ev[k + 1]) * 1e-3 for k in range(steps))
+    out = {"total_s": total, "mean_s": total / steps, "median_s": per[len(per) // 2], "best_s": per[0],
+           "launches": steps * h.launches_per_call, "n_buffers": n_buf, "handle": h, "bufs": bufs, "vis": vis}
+    return out
+
+
+def time_e2e(pkg, torch, w, h, steps, rank=0):
+    """Same metric through the public call with HOST buffers: per step, H2D of the integration from
+    pinned memory, corr_xengine, D2H of the visibilities -- all inside the timed region."""
+    n_host = 2 if w.in_bytes > (1 << 28) else 4
+    host = [torch.from_numpy(w.generate(integration=50 + k + 1000 * rank)).pin_memory() for k in range(n_host)]
+    d_in = torch.empty_like(host[0], device="cuda")
+    vis = h.empty_vis()
+    h_vis = torch.empty(vis.shape, dtype=vis.dtype).pin_memory()
+    stream = torch.cuda.current_stream()
+    for k in range(2):
+        d_in.copy_(host[k % n_host], non_blocking=True)
+        h.xengine(d_in, vis, stream)
+        h_vis.copy_(vis, non_blocking=True)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for k in range(steps):
+        d_in.copy_(host[k % n_host], non_blocking=True)
+        h.xengine(d_in, vis, stream)
+        h_vis.copy_(vis, non_blocking=True)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / steps
+    return {"value": w.cmacs / sec, "unit": UNIT, "h2d_bytes_per_step": w.in_bytes, "d2h_bytes_per_step": w.vis_bytes,
+            "ms_per_step": sec * 1e3, "steps": steps, "h2d_gbs": w.in_bytes / sec / 1e9}
+
+
+def cpu_baseline(w, target_s=12.0, gpu_vis=None):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the SAME
+    workload: the first k channels over the full integration (channels are independent,
+    PAPER.md:115).  Also compares those channels with the GPU output of the timed run."""
+    import numpy as np
+    import oracle
+    cores = oracle.host_threads()
+    fn = oracle.xengine_ci8 if w.dtype == "ci8" else oracle.xengine_cf32
+    x = w.generate()
+    t0 = time.perf_counter()
+    fn(x, 0, 1, threads=1)
+    one = max(time.perf_counter() - t0, 1e-4)            # one channel, one thread
+    k = int(max(cores, min(w.n_chan, target_s * cores / one)))
+    k = min(w.n_chan, k)
+    t0 = time.perf_counter()
+    ref = fn(x, 0, k, threads=cores)
+    sec = time.perf_counter() - t0
+    out = {"value": w.n_time * k * w.n_baselines / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"channels 0..{k - 1} of {w.n_chan}, all T={w.n_time} samples, {sec:.1f} s, OpenMP over channels"}
+    if gpu_vis is not None:
+        g = gpu_vis[:k]
+        if w.dtype == "ci8":
+            out["parity"] = "bit-exact" if np.array_equal(g, ref) else "MISMATCH"
+        else:
+            N = w.n_inputs
+            ii, jj = np.tril_indices(N)
+            sc = np.sqrt(np.abs(ref[:, ii * (ii + 1) // 2 + ii, 0] * ref[:, jj * (jj + 1) // 2 + jj, 0]))
+            err = np.hypot(g[..., 0] - ref[..., 0], g[..., 1] - ref[..., 1])
+            worst = float(np.max(err / np.maximum(sc, 1e-300)))
+            out["parity"] = f"max err/scale {worst:.2e} (tol 1e-5)" if worst <= 1e-5 else f"OUT OF TOLERANCE {worst:.2e}"
+    return out
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on the host cores; each step a bounded sample of the workload."""
+    import oracle
+    cores = oracle.host_threads()
+    fn = oracle.xengine_ci8 if w.dtype == "ci8" else oracle.xengine_cf32
+    x = w.generate()
+    t0 = time.perf_counter()
+    fn(x, 0, 1, threads=1)
+    one = max(time.perf_counter() - t0, 1e-4)
+    k = int(min(w.n_chan, max(cores, 2.0 * cores / one)))   # about 2 s of work per step
+    for _ in range(args.warmup):
+        fn(x, 0, k, threads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        fn(x, 0, k, threads=cores)
+    sec = (time.perf_counter() - t0) / args.steps
+    val = w.n_time * k * w.n_baselines / sec
+    sample = f"channels 0..{k - 1} of {w.n_chan}, all T={w.n_time} samples per step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int64" if w.dtype == "ci8" else "f64", "data": "synthetic",
+            "config": {"workload": workload_name(w)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(w):
+    return (f"{w.name}: N_I={w.n_inputs}, {w.n_chan} channels, T={w.n_time}, "
+            f"{'complex int8 -> int32' if w.dtype == 'ci8' else 'complex float32'}, 1 integration per step")
+
+
+def dist_setup(n_gpus):
+    """One process per GPU under torchrun; returns (rank, world, dist or None)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, None
+    import torch
+    import torch.distributed as dist
+    rank, local = int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
+    if torch.cuda.is_available():
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        dist.init_process_group("gloo")
+    return rank, world, dist
+
+
+def reduce_max(dist, value, device):
+    """Max over ranks of a python float (the job is as slow as its slowest rank)."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
+    """Kernel-only numbers of another config (context for 'vs N_I'; not a bench line of its own)."""
+    import corrgen
+    w = corrgen.CONFIGS[key]
+    r = time_config(pkg, torch, w, steps, warmup)
+    t_a, t_b = roofline_times(w, peaks)
+    sec = r["median_s"]
+    out = {"n_inputs": w.n_inputs, "value": w.cmacs / sec, "unit": UNIT, "ms": sec * 1e3,
+           "bound": "hbm" if t_a >= t_b else ("tensor" if w.dtype == "ci8" else "alu"),
+           "roofline_ms": max(t_a, t_b) * 1e3, "frac": max(t_a, t_b) / sec, "n_buffers": r["n_buffers"]}
+    r["handle"].destroy()
+    del r
+    torch.cuda.empty_cache()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="c2")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=8)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    import corrgen
+    w = corrgen.CONFIGS[args.config]
+    rank0 = int(os.environ.get("RANK", "0")) == 0
+    if args.impl == "reference":
+        if rank0:
+            run_reference(args, w)
+        return
+
+    import torch
+    import paper_0906_1887_b200 as pkg
+    rank, world, dist = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    pkg.lib()
+    peaks = measured_peaks()
+    dev = torch.device("cuda", torch.cuda.current_device())
+
+    sampler = ClockSampler(index=torch.cuda.current_device()) if rank == 0 else None
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    r = time_config(pkg, torch, w, args.steps, args.warmup, rank, sampler)
+    if dist is not None:
+        dist.barrier()
+    total_s = reduce_max(dist, r["total_s"], dev)
+    sec = total_s / args.steps
+    h = r["handle"]
+    if r["n_buffers"] > 1:
+        h.xengine(r["bufs"][0], r["vis"])
+        torch.cuda.synchronize()
+    gpu_vis = r["vis"].cpu().numpy()
+
+    e2e = time_e2e(pkg, torch, w, h, args.e2e_steps, rank)
+    e2e_sec = reduce_max(dist, e2e["ms_per_step"] * 1e-3, dev)
+    e2e["value"] = world * w.cmacs / e2e_sec
+    e2e["ms_per_step"] = e2e_sec * 1e3
+
+    if rank != 0:
+        return
+    t_a, t_b = roofline_times(w, peaks)
+    kern = r["median_s"]
+    if t_a >= t_b:
+        roof = {"bound": "hbm", "achieved": w.in_bytes / kern / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    elif w.dtype == "ci8":
+        roof = {"bound": "tensor", "achieved": 8.0 * w.cmacs / kern / 1e12, "peak": 2.0 * peaks["bf16_tflops"], "unit": "TOP/s"}
+    else:
+        roof = {"bound": "alu", "achieved": 8.0 * w.cmacs / kern / 1e12, "peak": FP32_PEAK_FLOPS / 1e12, "unit": "TFLOP/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["peak_source"] = peaks["source"] + (" (int8 = 2 x measured bf16 burst, provisional)" if roof["bound"] == "tensor" else "")
+    roof["kernel"] = "xengine_i8_kernel" if w.dtype == "ci8" else "xengine_f32_kernel"
+    roof["kernel_ms"] = kern * 1e3
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = json.load(open(tpath)).get(args.config) if os.path.exists(tpath) else None
+    roof["traffic"] = traffic
+
+    line = {"metric": METRIC, "value": world * w.cmacs / sec, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "s8 x s8 -> s32" if w.dtype == "ci8" else "f32", "data": "synthetic",
+            "config": {"workload": workload_name(w), "n_inputs": w.n_inputs, "n_chan": w.n_chan, "n_time": w.n_time,
+                       "parallelism": f"channel-independent replicas x{world}" if world > 1 else "single GPU",
+                       "l2": (f"input {w.in_bytes / 1e6:.0f} MB per step > 126 MB L2, no flush needed" if r["n_buffers"] == 1
+                              else f"rotating {r['n_buffers']} distinct input buffers ({r['n_buffers'] * w.in_bytes / 1e6:.0f} MB > L2)")},
+            "clocks": sampler.summary() if sampler else None,
+            "e2e": e2e, "gpu_launches": r["launches"], "roofline": roof}
+    if not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(w, gpu_vis=gpu_vis)
+    del r
+    h.destroy()
+    torch.cuda.empty_cache()
+    if not args.no_sweep and world == 1:
+        sweep = {}
+        for key in ("c1", "c2", "c3", "c4", "c5"):
+            if key == args.config:
+                continue
+            try:
+                sweep[key] = sweep_entry(pkg, torch, key, peaks)
+            except Exception as e:  # the headline line must survive a failing side measurement
+                sweep[key] = {"error": str(e)[:200]}
+        line["by_config"] = sweep
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

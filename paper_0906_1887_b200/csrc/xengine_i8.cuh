@@ -105,7 +105,7 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap, const I8Params p) {
             const int panel = (l < nJ) ? (J0 + l) : I;
             if (p.turned)
               tma_load_3d(dst + l * panel_stage_bytes, &tmap, &full_bar[stage], panel * kPanelBytes, ks * p.bk,
-                          chan, pol);
+                          p.pair_mode ? (chan >> 1) : chan, pol);
             else
               tma_load_2d(dst + l * panel_stage_bytes, &tmap, &full_bar[stage], x0 + panel * kPanelBytes,
                           ks * p.bk, pol);
