@@ -95,6 +95,22 @@ int corr_launches_per_call(const corr_handle *h);
 int corr_set_turn(corr_handle *h, int mode);
 
 /*
+ * corr_set_probe -- DIAGNOSTICS ONLY (results are garbage while a probe is on): CI8 kernel with
+ * 1 = MMAs skipped (measures the TMA fill rate), 2 = TMA loads skipped (measures the MMA issue
+ * rate), 0 = normal.  Used by the roofline study in DESIGN.md, never by tests of results.
+ */
+int corr_set_probe(corr_handle *h, int mode);
+
+/*
+ * corr_probe_mma -- measures the tcgen05.mma.kind::i8 issue rate on the current device (the int8
+ * tensor peak the roofline needs; it is not in MEASURED_PEAKS.json).  M in {64,128}, N multiple of
+ * 16 <= 256, K = 32; mn_major = 1 for the operand layout the fused corner turn produces, 0 for
+ * K-major.  out[0] = kernel ms, out[1] = SM cycles per MMA, out[2] = dense TOP/s over all SMs.
+ * No global-memory traffic; shared-memory operands are zeros.
+ */
+int corr_probe_mma(int m, int n, int mn_major, int iters, double *out);
+
+/*
  * corr_corner_turn -- the standalone corner-turn kernel, CI8 or CF32:
  *   d_in  [T][C][N] samples  ->  d_out [C][T][N] samples (per-channel, time-major tiles),
  * 16-byte vectorised coalesced loads and stores through a shared-memory tile.  Pure byte

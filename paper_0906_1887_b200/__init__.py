@@ -18,7 +18,7 @@ CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
-           "corr_corner_turn", "corr_stream_run")
+           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma")
 
 _lib = None
 
@@ -47,6 +47,9 @@ def lib():
         L.corr_vis_bytes.restype, L.corr_vis_bytes.argtypes = ctypes.c_size_t, [vp]
         L.corr_launches_per_call.restype, L.corr_launches_per_call.argtypes = ci, [vp]
         L.corr_set_turn.restype, L.corr_set_turn.argtypes = ci, [vp, ci]
+        L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
+        L.corr_probe_mma.restype = ci
+        L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
         L.corr_stream_run.restype = ci
         L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
@@ -145,6 +148,14 @@ class Correlator:
         if rc != CORR_OK:
             _raise()
         return d_vis, {"wall_s": stats[0], "device_s": stats[1], "kernel_s": stats[2], "h2d_s": stats[3]}
+
+
+def probe_mma(m=128, n=256, mn_major=True, iters=4096):
+    """tcgen05 int8 MMA issue-rate probe -> {"ms", "cycles_per_mma", "tops"} (see corr_probe_mma)."""
+    out = (ctypes.c_double * 3)()
+    if lib().corr_probe_mma(m, n, 1 if mn_major else 0, iters, out) != CORR_OK:
+        _raise()
+    return {"ms": out[0], "cycles_per_mma": out[1], "tops": out[2]}
 
 
 def corr_create(n_inputs, n_chan, n_time, dtype):

@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "corner_turn.cuh"
+#include "probe_mma.cuh"
 #include "xengine_f32.cuh"
 #include "xengine_i8.cuh"
 
@@ -55,7 +56,7 @@ EncodeTiledFn encode_tiled_fn() {
 
 struct MapCacheEntry {
   const void *ptr;
-  CUtensorMap map;
+  CUtensorMap map[3];  // box heights 256, 128, 64 time rows
 };
 
 }  // namespace
@@ -66,12 +67,11 @@ struct corr_handle {
   size_t in_bytes, vis_bytes;
   int n_sms;
   int turn_mode;
+  int probe;
   // CI8 plan
-  int pair_mode, panels, bk, slots, stages, grid_i8;
+  int pair_mode, grid_i8;
   size_t smem_i8;
-  int4 *d_items_i8;
-  int *d_offsets_i8;
-  int n_items_i8;
+  corr::I8Params ip;  // schedule + problem, passed by value into the constant bank at each launch
   void *d_scratch;  // corner-turn output (standalone mode)
   std::vector<MapCacheEntry> maps;
   // CF32 plan
@@ -85,48 +85,61 @@ struct corr_handle {
 
 namespace {
 
-// Static balanced schedule: items in channel-major order (so that CTAs running at the same time
-// share a channel's panels in L2), each given to the least-loaded CTA so far.
-void plan_i8(corr_handle *h, std::vector<int4> &items, std::vector<int> &offsets) {
-  const int N = h->n_inputs;
+// Schedule planning (host side of the uniform decode in xengine_i8.cuh).
+void plan_i8(corr_handle *h) {
+  corr::I8Params &ip = h->ip;
+  memset(&ip, 0, sizeof ip);
+  const int N = h->n_inputs, C = h->n_chan, T = h->n_time;
   h->pair_mode = (N == 32) ? 1 : 0;
-  h->panels = h->pair_mode ? 1 : (2 * N + 127) / 128;
-  const int groups = h->pair_mode ? (h->n_chan + 1) / 2 : h->n_chan;
-  h->slots = h->panels <= 4 ? h->panels : 5;
-  h->bk = h->slots == 1 ? 256 : h->slots == 2 ? 128 : 64;
-  const size_t stage_bytes = static_cast<size_t>(h->slots) * h->bk * 128;
-  h->stages = static_cast<int>(std::min<size_t>(corr::kMaxStages, (220 * 1024) / stage_bytes));
-  h->smem_i8 = stage_bytes * h->stages + 1024;
-
-  struct Raw { int4 it; long long cost; };
-  std::vector<Raw> raw;
-  for (int g = 0; g < groups; ++g) {
-    const int chan = h->pair_mode ? 2 * g : g;
-    for (int I = h->panels - 1; I >= 0; --I)
+  const int panels_per_chan = h->pair_mode ? 1 : (2 * N + 127) / 128;
+  ip.n_time = T; ip.n_inputs = N; ip.n_chan = C; ip.pair_mode = h->pair_mode;
+  ip.n_baselines = h->n_baselines;
+  ip.diag = panels_per_chan == 1;
+  int max_load = 1;
+  if (ip.diag) {
+    ip.n_panels = h->pair_mode ? (C + 1) / 2 : C;
+    ip.n_groups = (ip.n_panels + 3) / 4;
+    ip.n_kinds = 1;
+    max_load = 4;
+    // split the integration into time slices until the grid is filled evenly
+    const int base = ip.n_groups, G = h->n_sms;
+    int best_s = 1;
+    double best_eff = 0.0;
+    for (int s = 1; s <= 64; ++s) {
+      int len = ((T + s - 1) / s + 63) / 64 * 64;
+      if (len < 128 && s > 1) break;
+      const int s_eff = (T + len - 1) / len;
+      if (s_eff != s) continue;
+      const long long n = 1LL * base * s;
+      const long long rounds = (n + G - 1) / G;
+      // load of the busiest CTA in units of samples vs the mean
+      const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
+      if (eff > best_eff + 0.02) { best_eff = eff; best_s = s; }
+      if (best_eff >= 0.95) break;
+    }
+    ip.n_slices = best_s;
+    ip.slice_len = best_s == 1 ? T : ((T + best_s - 1) / best_s + 63) / 64 * 64;
+  } else {
+    ip.n_panels = panels_per_chan;
+    ip.n_groups = C;
+    int k = 0;
+    for (int I = panels_per_chan - 1; I >= 0; --I)
       for (int J0 = 0; J0 <= I; J0 += 4) {
-        const int nJ = std::min(4, I - J0 + 1);
-        const bool a_in_b = I < J0 + nJ;
-        const long long cost = 2LL * h->n_time * nJ + 700LL * nJ + 64LL * h->n_time / 32 * (a_in_b ? 0 : 0) + 1500;
-        raw.push_back({make_int4(chan, I | (J0 << 16), nJ, 0), cost});
+        const int nblk = std::min(4, I - J0 + 1);
+        if (!(I < J0 + nblk)) max_load = 5;
+        else max_load = std::max(max_load, nblk);
+        ip.kinds[k++] = static_cast<unsigned>(I) | (static_cast<unsigned>(J0) << 8) | (static_cast<unsigned>(nblk) << 16);
       }
+    ip.n_kinds = k;
+    ip.n_slices = 1;
+    ip.slice_len = T;
   }
-  h->n_items_i8 = static_cast<int>(raw.size());
-  h->grid_i8 = std::min(h->n_items_i8, h->n_sms);
-  std::vector<std::vector<int4>> per(h->grid_i8);
-  typedef std::pair<long long, int> LB;  // (load, cta)
-  std::priority_queue<LB, std::vector<LB>, std::greater<LB>> pq;
-  for (int b = 0; b < h->grid_i8; ++b) pq.push({0, b});
-  for (const Raw &r : raw) {
-    LB lb = pq.top();
-    pq.pop();
-    per[lb.second].push_back(r.it);
-    pq.push({lb.first + r.cost, lb.second});
-  }
-  offsets.assign(1, 0);
-  for (int b = 0; b < h->grid_i8; ++b) {
-    items.insert(items.end(), per[b].begin(), per[b].end());
-    offsets.push_back(static_cast<int>(items.size()));
-  }
+  ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices;
+  ip.rot = ip.n_kinds > 1 ? 1 : 0;
+  ip.stage_bytes = (max_load == 5 ? 5 : 4) * 64 * 128;
+  ip.stages = std::min<int>(corr::kMaxStages, (232448 - 4096) / ip.stage_bytes);
+  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + 1024;
+  h->grid_i8 = std::min(ip.n_items, h->n_sms);
 }
 
 void plan_f32(corr_handle *h, std::vector<int2> &items) {
@@ -138,7 +151,7 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
   h->f32_threads = blocks == 1 ? 160 : corr::kF32Threads;  // 136 active tiles on a diagonal block
 }
 
-int encode_map(corr_handle *h, const void *base, bool turned, CUtensorMap *out) {
+int encode_map(corr_handle *h, const void *base, bool turned, int box_rows, CUtensorMap *out) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return fail(CORR_ECUDA, "cuTensorMapEncodeTiled entry point not available");
   const cuuint64_t row = static_cast<cuuint64_t>(2) * h->n_inputs;  // bytes per (t, c)
@@ -146,7 +159,7 @@ int encode_map(corr_handle *h, const void *base, bool turned, CUtensorMap *out) 
   if (!turned) {
     cuuint64_t dims[2] = {row * h->n_chan, static_cast<cuuint64_t>(h->n_time)};
     cuuint64_t strides[1] = {row * h->n_chan};
-    cuuint32_t box[2] = {128, static_cast<cuuint32_t>(h->bk)};
+    cuuint32_t box[2] = {128, static_cast<cuuint32_t>(box_rows)};
     cuuint32_t es[2] = {1, 1};
     r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), dims, strides, box, es,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -156,7 +169,7 @@ int encode_map(corr_handle *h, const void *base, bool turned, CUtensorMap *out) 
     const cuuint64_t groups = h->pair_mode ? h->n_chan / 2 : h->n_chan;
     cuuint64_t dims[3] = {grow, static_cast<cuuint64_t>(h->n_time), groups};
     cuuint64_t strides[2] = {grow, grow * h->n_time};
-    cuuint32_t box[3] = {128, static_cast<cuuint32_t>(h->bk), 1};
+    cuuint32_t box[3] = {128, static_cast<cuuint32_t>(box_rows), 1};
     cuuint32_t es[3] = {1, 1, 1};
     r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(base), dims, strides, box, es,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -168,14 +181,17 @@ int encode_map(corr_handle *h, const void *base, bool turned, CUtensorMap *out) 
 
 int get_map(corr_handle *h, const void *base, bool turned, const CUtensorMap **out) {
   for (const MapCacheEntry &e : h->maps)
-    if (e.ptr == base) { *out = &e.map; return CORR_OK; }
+    if (e.ptr == base) { *out = e.map; return CORR_OK; }
   if (h->maps.size() >= 64) h->maps.erase(h->maps.begin());
   MapCacheEntry e;
   e.ptr = base;
-  int rc = encode_map(h, base, turned, &e.map);
-  if (rc != CORR_OK) return rc;
+  const int rows[3] = {256, 128, 64};
+  for (int m = 0; m < 3; ++m) {
+    int rc = encode_map(h, base, turned, rows[m], &e.map[m]);
+    if (rc != CORR_OK) return rc;
+  }
   h->maps.push_back(e);
-  *out = &h->maps.back().map;
+  *out = h->maps.back().map;
   return CORR_OK;
 }
 
@@ -234,8 +250,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->vis_bytes = static_cast<size_t>(n_chan) * h->n_baselines * 8;
   h->n_sms = prop.multiProcessorCount;
   h->turn_mode = CORR_TURN_FUSED;
-  h->d_items_i8 = nullptr;
-  h->d_offsets_i8 = nullptr;
+  h->probe = 0;
   h->d_items_f32 = nullptr;
   h->d_scratch = nullptr;
   h->d_stream_in[0] = h->d_stream_in[1] = nullptr;
@@ -243,15 +258,8 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
 
   cudaError_t e = cudaSuccess;
   if (dtype == CORR_CI8) {
-    std::vector<int4> items;
-    std::vector<int> offsets;
-    plan_i8(h, items, offsets);
-    e = cudaMalloc(&h->d_items_i8, items.size() * sizeof(int4));
-    if (e == cudaSuccess) e = cudaMalloc(&h->d_offsets_i8, offsets.size() * sizeof(int));
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_items_i8, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_offsets_i8, offsets.data(), offsets.size() * sizeof(int), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
+    plan_i8(h);
+    e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
   } else {
     std::vector<int2> items;
     plan_f32(h, items);
@@ -268,8 +276,6 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
 
 int corr_destroy(corr_handle *h) {
   if (!h) return CORR_OK;
-  cudaFree(h->d_items_i8);
-  cudaFree(h->d_offsets_i8);
   cudaFree(h->d_items_f32);
   cudaFree(h->d_scratch);
   cudaFree(h->d_stream_in[0]);
@@ -284,7 +290,49 @@ size_t corr_in_bytes(const corr_handle *h) { return h ? h->in_bytes : 0; }
 size_t corr_vis_bytes(const corr_handle *h) { return h ? h->vis_bytes : 0; }
 int corr_launches_per_call(const corr_handle *h) {
   if (!h) return 0;
-  return (h->dtype == CORR_CI8 && h->turn_mode == CORR_TURN_STANDALONE) ? 2 : 1;
+  return (h->dtype == CORR_CI8 && h->turn_mode == CORR_TURN_STANDALONE) ? 2 : 1;  // kernels; a memset node precedes them when the integration is time-sliced
+}
+
+int corr_probe_mma(int m, int n, int mn_major, int iters, double *out) {
+  if ((m != 64 && m != 128) || n < 16 || n > 256 || (n % 16) || iters < 16 || !out)
+    return fail(CORR_EINVAL, "corr_probe_mma: bad argument");
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  unsigned long long *d_cyc = nullptr;
+  CUDA_TRY(cudaMalloc(&d_cyc, sms * sizeof(unsigned long long)));
+  corr::ProbeParams pp{iters, m, n, mn_major, d_cyc};
+  const int smem = 49 * 1024 + 1024;
+  CUDA_TRY(cudaFuncSetAttribute(corr::probe_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  corr::probe_mma_kernel<<<sms, 128, smem>>>(pp);  // warm-up
+  cudaEventRecord(e0);
+  corr::probe_mma_kernel<<<sms, 128, smem>>>(pp);
+  cudaEventRecord(e1);
+  cudaError_t e = cudaDeviceSynchronize();
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  std::vector<unsigned long long> cyc(sms);
+  cudaMemcpy(cyc.data(), d_cyc, sms * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+  cudaFree(d_cyc);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (e != cudaSuccess) return fail(CORR_ECUDA, "corr_probe_mma: %s", cudaGetErrorString(e));
+  double mean = 0;
+  for (unsigned long long c : cyc) mean += static_cast<double>(c);
+  mean /= sms;
+  out[0] = ms;
+  out[1] = mean / iters;
+  out[2] = 2.0 * m * n * 32.0 * iters * sms / (ms * 1e-3) / 1e12;
+  return CORR_OK;
+}
+
+int corr_set_probe(corr_handle *h, int mode) {
+  if (!h) return fail(CORR_EINVAL, "corr_set_probe: NULL handle");
+  h->probe = mode;
+  return CORR_OK;
 }
 
 int corr_set_turn(corr_handle *h, int mode) {
@@ -364,20 +412,12 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   const CUtensorMap *map = nullptr;
   int rc = get_map(h, src, turned, &map);
   if (rc != CORR_OK) return rc;
-  corr::I8Params ip;
-  ip.items = h->d_items_i8;
-  ip.offsets = h->d_offsets_i8;
-  ip.n_time = h->n_time;
-  ip.n_inputs = h->n_inputs;
-  ip.n_chan = h->n_chan;
-  ip.pair_mode = h->pair_mode;
-  ip.bk = h->bk;
-  ip.slots = h->slots;
-  ip.stages = h->stages;
+  corr::I8Params ip = h->ip;
   ip.turned = turned ? 1 : 0;
-  ip.n_baselines = h->n_baselines;
   ip.vis = static_cast<int2 *>(d_vis);
-  corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(*map, ip);
+  ip.probe = h->probe;
+  if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
+  corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }

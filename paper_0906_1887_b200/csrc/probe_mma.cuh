@@ -1,0 +1,60 @@
+// probe_mma.cuh -- tcgen05.mma.kind::i8 issue-rate probe (the int8 tensor peak is
+// not in MEASURED_PEAKS.json, so it is measured here).  One CTA per SM; one thread issues `iters`
+// back-to-back MMAs on zero-filled shared-memory operands (values do not matter for timing) into
+// two alternating TMEM accumulators, then commits and waits.  No global traffic at all.
+#pragma once
+#include "ptx_sm100.cuh"
+
+namespace corr {
+
+struct ProbeParams {
+  int iters;
+  int m, n;        // MMA shape (M = 64 | 128, N multiple of 16 up to 256), K = 32
+  int mn_major;    // 1: both operands MN-major (what the fused corner turn produces); 0: K-major
+  unsigned long long *cycles;  // [gridDim.x] elapsed SM cycles of the issue loop
+};
+
+__global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) {
+  extern __shared__ __align__(1024) uint8_t psmem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(psmem_raw) + 1023) & ~uintptr_t(1023));
+  __shared__ __align__(8) uint64_t done_bar;
+  __shared__ uint32_t tmem_base_smem;
+  // operands: A at 0 (16 KB = 128 x 128 B), B at 16 KB (32 KB = 256 x 128 B)
+  for (int i = threadIdx.x; i < 48 * 1024 / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+  if (threadIdx.x == 0) {
+    mbar_init(&done_bar, 1);
+    fence_mbar_init();
+  }
+  fence_proxy_async();
+  if (threadIdx.x < 32) tmem_alloc(&tmem_base_smem, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+  if (threadIdx.x == 0) {
+    const uint32_t a0 = smem_u32(smem), b0 = a0 + 16 * 1024;
+    uint32_t idesc = idesc_i8_mn(p.m, p.n);
+    if (!p.mn_major) idesc &= ~((1u << 15) | (1u << 16));
+    const long long t0 = clock64();
+    for (int it = 0; it < p.iters; ++it) {
+      const int k = it & 3;
+      // MN-major: 32 k-rows of 128 B per MMA -> +4096 B; K-major: 32 B of each 128-B row -> +32 B
+      const uint32_t off = p.mn_major ? k * 4096 : k * 32;
+      const uint64_t a_desc = smem_desc_mn_sw128(a0 + off, 16 * 1024, 1024);
+      const uint64_t b_desc = smem_desc_mn_sw128(b0 + off, 16 * 1024, 1024);
+      mma_i8_ss(tmem_base + ((it >> 2) & 1) * 256, a_desc, b_desc, idesc, it >= 8);
+    }
+    mma_commit(&done_bar);
+    mbar_wait(&done_bar, 0);
+    const long long t1 = clock64();
+    p.cycles[blockIdx.x] = static_cast<unsigned long long>(t1 - t0);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+}  // namespace corr
