@@ -105,7 +105,8 @@ int corr_set_probe(corr_handle *h, int mode);
  * corr_probe_mma -- measures the tcgen05.mma.kind::i8 issue rate on the current device (the int8
  * tensor peak the roofline needs; it is not in MEASURED_PEAKS.json).  M in {64,128}, N multiple of
  * 16 <= 256, K = 32; mn_major = 1 for the operand layout the fused corner turn produces, 0 for
- * K-major.  out[0] = kernel ms, out[1] = SM cycles per MMA, out[2] = dense TOP/s over all SMs.
+ * K-major (add 2 for pseudo-random instead of zero operand bytes).  out[0] = kernel ms, out[1] = SM
+ * cycles per MMA, out[2] = dense TOP/s over all SMs, out[3] = effective SM MHz during the loop.
  * No global-memory traffic; shared-memory operands are zeros.
  */
 int corr_probe_mma(int m, int n, int mn_major, int iters, double *out);

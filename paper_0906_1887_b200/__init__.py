@@ -150,12 +150,12 @@ class Correlator:
         return d_vis, {"wall_s": stats[0], "device_s": stats[1], "kernel_s": stats[2], "h2d_s": stats[3]}
 
 
-def probe_mma(m=128, n=256, mn_major=True, iters=4096):
-    """tcgen05 int8 MMA issue-rate probe -> {"ms", "cycles_per_mma", "tops"} (see corr_probe_mma)."""
-    out = (ctypes.c_double * 3)()
-    if lib().corr_probe_mma(m, n, 1 if mn_major else 0, iters, out) != CORR_OK:
+def probe_mma(m=128, n=256, mn_major=True, iters=4096, random_fill=False):
+    """tcgen05 int8 MMA issue-rate probe (see corr_probe_mma)."""
+    out = (ctypes.c_double * 4)()
+    if lib().corr_probe_mma(m, n, (1 if mn_major else 0) | (2 if random_fill else 0), iters, out) != CORR_OK:
         _raise()
-    return {"ms": out[0], "cycles_per_mma": out[1], "tops": out[2]}
+    return {"ms": out[0], "cycles_per_mma": out[1], "tops": out[2], "sm_mhz": out[3]}
 
 
 def corr_create(n_inputs, n_chan, n_time, dtype):

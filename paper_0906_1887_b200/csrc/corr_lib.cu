@@ -294,15 +294,17 @@ int corr_launches_per_call(const corr_handle *h) {
 }
 
 int corr_probe_mma(int m, int n, int mn_major, int iters, double *out) {
+  const int fill = mn_major >> 1;  // bit 1 of mn_major: pseudo-random operand bytes; bits 2,3: A == B, wide smem walk
+  mn_major &= 1;
   if ((m != 64 && m != 128) || n < 16 || n > 256 || (n % 16) || iters < 16 || !out)
     return fail(CORR_EINVAL, "corr_probe_mma: bad argument");
   int dev = 0, sms = 0;
   CUDA_TRY(cudaGetDevice(&dev));
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   unsigned long long *d_cyc = nullptr;
-  CUDA_TRY(cudaMalloc(&d_cyc, sms * sizeof(unsigned long long)));
-  corr::ProbeParams pp{iters, m, n, mn_major, d_cyc};
-  const int smem = 49 * 1024 + 1024;
+  CUDA_TRY(cudaMalloc(&d_cyc, 2 * sms * sizeof(unsigned long long)));
+  corr::ProbeParams pp{iters, m, n, fill, mn_major, d_cyc};
+  const int smem = 225 * 1024;
   CUDA_TRY(cudaFuncSetAttribute(corr::probe_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
@@ -314,18 +316,20 @@ int corr_probe_mma(int m, int n, int mn_major, int iters, double *out) {
   cudaError_t e = cudaDeviceSynchronize();
   float ms = 0.f;
   cudaEventElapsedTime(&ms, e0, e1);
-  std::vector<unsigned long long> cyc(sms);
-  cudaMemcpy(cyc.data(), d_cyc, sms * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+  std::vector<unsigned long long> cyc(2 * sms);
+  cudaMemcpy(cyc.data(), d_cyc, 2 * sms * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
   cudaFree(d_cyc);
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   if (e != cudaSuccess) return fail(CORR_ECUDA, "corr_probe_mma: %s", cudaGetErrorString(e));
-  double mean = 0;
-  for (unsigned long long c : cyc) mean += static_cast<double>(c);
+  double mean = 0, ns = 0;
+  for (int b = 0; b < sms; ++b) { mean += static_cast<double>(cyc[2 * b]); ns += static_cast<double>(cyc[2 * b + 1]); }
   mean /= sms;
+  ns /= sms;
   out[0] = ms;
   out[1] = mean / iters;
-  out[2] = 2.0 * m * n * 32.0 * iters * sms / (ms * 1e-3) / 1e12;
+  out[2] = 2.0 * m * n * 32.0 * iters * sms / (ns * 1e-9) / 1e12;  // over the issue loop itself
+  out[3] = mean / ns * 1e3;                                        // effective SM MHz during the loop
   return CORR_OK;
 }
 

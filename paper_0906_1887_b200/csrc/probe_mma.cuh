@@ -10,8 +10,9 @@ namespace corr {
 struct ProbeParams {
   int iters;
   int m, n;        // MMA shape (M = 64 | 128, N multiple of 16 up to 256), K = 32
+  int fill;        // 0: zero operands, 1: pseudo-random bytes (power draw differs, timing should not)
   int mn_major;    // 1: both operands MN-major (what the fused corner turn produces); 0: K-major
-  unsigned long long *cycles;  // [gridDim.x] elapsed SM cycles of the issue loop
+  unsigned long long *cycles;  // [2*gridDim.x]: elapsed SM cycles, elapsed globaltimer ns of the issue loop
 };
 
 __global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) {
@@ -20,7 +21,10 @@ __global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) 
   __shared__ __align__(8) uint64_t done_bar;
   __shared__ uint32_t tmem_base_smem;
   // operands: A at 0 (16 KB = 128 x 128 B), B at 16 KB (32 KB = 256 x 128 B)
-  for (int i = threadIdx.x; i < 48 * 1024 / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = threadIdx.x; i < 48 * 1024 / 16; i += blockDim.x) {
+    const uint32_t v = (p.fill & 1) ? (i * 2654435761u + blockIdx.x * 40503u) : 0u;
+    reinterpret_cast<uint4 *>(smem)[i] = make_uint4(v, v * 3u + 1u, v ^ 0x9E3779B9u, v * 7u);
+  }
   if (threadIdx.x == 0) {
     mbar_init(&done_bar, 1);
     fence_mbar_init();
@@ -35,19 +39,27 @@ __global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) 
     const uint32_t a0 = smem_u32(smem), b0 = a0 + 16 * 1024;
     uint32_t idesc = idesc_i8_mn(p.m, p.n);
     if (!p.mn_major) idesc &= ~((1u << 15) | (1u << 16));
+    unsigned long long g0, g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
     const long long t0 = clock64();
     for (int it = 0; it < p.iters; ++it) {
       const int k = it & 3;
       // MN-major: 32 k-rows of 128 B per MMA -> +4096 B; K-major: 32 B of each 128-B row -> +32 B
-      const uint32_t off = p.mn_major ? k * 4096 : k * 32;
+      uint32_t off = p.mn_major ? k * 4096 : k * 32;
+      if (p.fill & 4) off = (it % 40) * 4096;  // walk over 160 KB of shared memory instead of 16 KB
       const uint64_t a_desc = smem_desc_mn_sw128(a0 + off, 16 * 1024, 1024);
-      const uint64_t b_desc = smem_desc_mn_sw128(b0 + off, 16 * 1024, 1024);
-      mma_i8_ss(tmem_base + ((it >> 2) & 1) * 256, a_desc, b_desc, idesc, it >= 8);
+      const uint64_t b_desc = (p.fill & 2) ? a_desc : smem_desc_mn_sw128(b0 + off, 16 * 1024, 1024);
+      uint32_t d = tmem_base + ((it >> 2) & 1) * 256;
+      if (p.fill & 8) d = tmem_base + (it & 3) * 128;           // D rotates over four 128-column blocks
+      if (p.fill & 16) d = tmem_base + (it & 1) * 256;          // D alternates between two 256-column chunks
+      mma_i8_ss(d, a_desc, b_desc, idesc, it >= 8);
     }
     mma_commit(&done_bar);
     mbar_wait(&done_bar, 0);
     const long long t1 = clock64();
-    p.cycles[blockIdx.x] = static_cast<unsigned long long>(t1 - t0);
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+    p.cycles[2 * blockIdx.x] = static_cast<unsigned long long>(t1 - t0);
+    p.cycles[2 * blockIdx.x + 1] = g1 - g0;
   }
   tc_fence_before();
   __syncthreads();

@@ -81,7 +81,11 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
       uint32_t ring = 0;  // accumulator ring entries handed out so far
       constexpr uint32_t kIdesc128 = idesc_i8_mn(128, 128), kIdesc256 = idesc_i8_mn(128, 256);
       constexpr uint32_t kDescHi = static_cast<uint32_t>(((1024ull >> 4) | (1ull << 14) | (2ull << 29)));
-      const uint32_t smem_lo = (smem_u32(smem) & 0x3FFFFu) >> 4;
+      const uint32_t smem_lo = __reduce_or_sync(0xffffffffu, (smem_u32(smem) & 0x3FFFFu) >> 4);
+      // REDUX lands in a uniform register: keeps the TMEM addresses out of the vector file (no R2UR per MMA)
+      const uint32_t tmem_u = __reduce_or_sync(0xffffffffu, tmem_base);
+      const long long dbg_t0 = clock64();
+      int dbg_n = 0;
       for (int r = 0; r < n_rounds; ++r) {
         const int g = item_of_round(p, r);
         if (g >= p.n_items) continue;
@@ -92,17 +96,18 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
         if (!(p.probe & 4))
           for (int q = 0; q < n_chunks; ++q) mbar_wait(&acc_empty[(ring + q) & 1], (((ring + q) >> 1) & 1) ^ 1);
         tc_fence_after();
-        const uint32_t d0 = tmem_base + (ring & 1) * kAccCols;        // chunk 0
-        const uint32_t d1 = tmem_base + ((ring + 1) & 1) * kAccCols;  // chunk 1
-        uint32_t acc = 0;
+        const uint32_t d0 = tmem_u + (ring & 1) * kAccCols;        // chunk 0
+        uint32_t d1 = tmem_u + ((ring + 1) & 1) * kAccCols;  // chunk 1
+        if (p.probe & 64) d1 = d0;
         for (int t = it.t0; t < it.t1; t += it.bk) {
           if (!(p.probe & 8)) mbar_wait(&full_bar[stage], phase);
-          tc_fence_after();
+          if (!(p.probe & 32)) tc_fence_after();
           const uint32_t lo_stage = (smem_lo + static_cast<uint32_t>(stage) * (p.stage_bytes >> 4)) | lbo_field;
           const int nk = (min(it.bk, it.t1 - t) + 31) >> 5;  // K = 32 samples per MMA; TMA zero-fills past T
           if (leader) {
             for (int k = 0; k < ((p.probe & 1) ? 0 : nk); ++k) {
               const uint32_t lo_k = lo_stage + static_cast<uint32_t>(k) * (32 * kPanelBytes / 16);
+              const uint32_t acc = (t != it.t0 || k != 0) ? 1u : 0u;  // uniform: first MMA of the slice overwrites
               if (p.diag) {
                 for (int b = 0; b < it.nblk; ++b) {
                   const uint64_t d = (static_cast<uint64_t>(kDescHi) << 32) | (lo_k + b * panel16);
@@ -117,11 +122,10 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
                   mma_i8_ss(d1, a_desc, b_desc1, it.nblk == 4 ? kIdesc256 : kIdesc128, acc);
                 }
               }
-              acc = 1;
+              ++dbg_n;
             }
             if (!(p.probe & 8)) mma_commit(&empty_bar[stage]);  // frees the smem stage when these MMAs retire
           }
-          acc = 1;
           __syncwarp();
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
         }
@@ -130,6 +134,8 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
         __syncwarp();
         ring += n_chunks;
       }
+      if ((p.probe & 128) && leader && blockIdx.x < 8)
+        p.vis[blockIdx.x] = make_int2(static_cast<int>(clock64() - dbg_t0), dbg_n);
     }
   } else if (warp >= 4 && !(p.probe & 4)) {
     // ===================================================================== epilogue
