@@ -124,11 +124,10 @@ void plan_i8(corr_handle *h) {
     ip.n_groups = C;
     int k = 0;
     for (int I = panels_per_chan - 1; I >= 0; --I)
-      for (int J0 = 0; J0 <= I; J0 += 4) {
-        const int nblk = std::min(4, I - J0 + 1);
-        if (!(I < J0 + nblk)) max_load = 5;
-        else max_load = std::max(max_load, nblk);
-        ip.kinds[k++] = static_cast<unsigned>(I) | (static_cast<unsigned>(J0) << 8) | (static_cast<unsigned>(nblk) << 16);
+      for (int J0 = 0; J0 <= I; J0 += 2) {
+        const int nblk = std::min(2, I - J0 + 1);
+        max_load = std::max(max_load, (I < J0 + nblk) ? nblk : nblk + 1);
+        ip.kinds[k++] = static_cast<unsigned short>(I | ((J0 >> 1) << 6) | ((nblk - 1) << 11));
       }
     ip.n_kinds = k;
     ip.n_slices = 1;
@@ -136,10 +135,13 @@ void plan_i8(corr_handle *h) {
   }
   ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices;
   ip.rot = ip.n_kinds > 1 ? 1 : 0;
-  ip.stage_bytes = (max_load == 5 ? 5 : 4) * 64 * 128;
-  ip.stages = std::min<int>(corr::kMaxStages, (232448 - 4096) / ip.stage_bytes);
-  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + 1024;
+  ip.stage_bytes = 4 * 64 * 128;  // 32 KB: 1 x 256, 2 x 128 or 3-4 x 64 time rows of 128 B
+  const int epi_bytes = corr::kEpiWarps * corr::kEpiWarpBytes;  // epilogue staging behind the stage ring
+  ip.stages = std::min<int>(corr::kMaxStages, (232448 - 4096 - epi_bytes) / ip.stage_bytes);
+  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + epi_bytes + 1024;
   h->grid_i8 = std::min(ip.n_items, h->n_sms);
+  const int deltas[2] = {h->grid_i8 + ip.rot, ip.rot};
+  for (int w = 0; w < 2; ++w) { ip.dq[w] = deltas[w] / ip.n_kinds; ip.dr[w] = deltas[w] % ip.n_kinds; }
 }
 
 void plan_f32(corr_handle *h, std::vector<int2> &items) {

@@ -47,8 +47,10 @@ __global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) 
       // MN-major: 32 k-rows of 128 B per MMA -> +4096 B; K-major: 32 B of each 128-B row -> +32 B
       uint32_t off = p.mn_major ? k * 4096 : k * 32;
       if (p.fill & 4) off = (it % 40) * 4096;  // walk over 160 KB of shared memory instead of 16 KB
-      const uint64_t a_desc = smem_desc_mn_sw128(a0 + off, 16 * 1024, 1024);
-      const uint64_t b_desc = (p.fill & 2) ? a_desc : smem_desc_mn_sw128(b0 + off, 16 * 1024, 1024);
+      const uint32_t lbo = (p.fill & 32) ? 8 * 1024 : 16 * 1024;  // second 128-byte block of an N = 256 operand
+      if (p.fill & 32) off = (it & 1) * 4096;
+      const uint64_t a_desc = smem_desc_mn_sw128(a0 + off, lbo, 1024);
+      const uint64_t b_desc = (p.fill & 2) ? a_desc : smem_desc_mn_sw128(b0 + off, lbo, 1024);
       uint32_t d = tmem_base + ((it >> 2) & 1) * 256;
       if (p.fill & 8) d = tmem_base + (it & 3) * 128;           // D rotates over four 128-column blocks
       if (p.fill & 16) d = tmem_base + (it & 1) * 256;          // D alternates between two 256-column chunks

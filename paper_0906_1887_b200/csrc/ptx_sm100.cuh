@@ -150,3 +150,23 @@ __host__ __device__ constexpr uint32_t idesc_i8_mn(uint32_t M, uint32_t N) {
 }
 
 }  // namespace corr
+
+// ----------------------------------------------------------------------------- bulk async stores
+namespace corr {
+// shared::cta -> global, 16-byte aligned on both sides, size a multiple of 16; joins the bulk async-group
+__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes)
+               : "memory");
+}
+// same, but global[i] += shared[i] on 32-bit signed integers (exact, order-independent)
+__device__ __forceinline__ void bulk_reduce_add_s32(void *gdst, const void *ssrc, uint32_t bytes) {
+  asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(gdst),
+               "r"(smem_u32(ssrc)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// wait until the shared-memory sources of all committed groups have been read (buffer reusable)
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// wait until all committed groups have completed (writes performed)
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+}  // namespace corr

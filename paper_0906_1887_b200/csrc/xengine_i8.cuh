@@ -7,7 +7,8 @@
 // blocks of G over a time slice in TMEM (int32) and folds them to complex visibilities
 //   Re V_ij = G[2i][2j] + G[2i+1][2j+1],  Im V_ij = G[2i+1][2j] - G[2i][2j+1].
 // Two item kinds:
-//   slab  (N_I >= 128): row panel I x column panels J0..J0+nblk-1 (<= I) of one channel;
+//   slab  (N_I >= 128): row panel I x column panels J0, J0+1 (<= I) of one channel: one 128x256
+//                       accumulator, so the two TMEM halves double-buffer items (epilogue overlaps MMA);
 //   diag  (N_I <= 64) : the diagonal blocks of up to four ADJACENT channels (or channel pairs), so
 //                       that each time row is fetched as one 512-byte contiguous run (HBM-friendly).
 // The schedule (descendant of the paper's constant-memory pair table) lives in the
@@ -20,7 +21,7 @@
 //            canonical MN-major operand tile, so the input is read from HBM exactly once.
 //   warp 1   MMA issuer (one thread): tcgen05.mma.kind::i8, M=128, N=128|256, K=32.
 //   warp 2   TMEM allocator.
-//   warps 4-7 epilogue: tcgen05.ld, 2x2 fold via shfl.xor 1, packed-triangle stores (or integer
+//   warps 4-11 epilogue (two per TMEM lane quadrant, one per half block): tcgen05.ld, 2x2 fold via shfl.xor 1, packed-triangle stores (or integer
 //            red.add when an integration is split into time slices; integer sums are exact and
 //            order-independent, so the result stays bit-exact).
 #pragma once
@@ -28,11 +29,12 @@
 
 namespace corr {
 
-constexpr int kI8Threads = 256;
+constexpr int kI8Threads = 384;    // 4 control warps + 8 epilogue warps
+constexpr int kEpiWarps = 8;
 constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64 complex int8 samples
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
 constexpr int kMaxStages = 8;
-constexpr int kMaxKinds = 544;    // slab kinds per channel at N_I = 4096
+constexpr int kMaxKinds = 1056;   // slab kinds per channel at N_I = 4096 (64 panels, column pairs)
 
 struct I8Params {
   // ---- schedule (uniform) ----
@@ -42,6 +44,7 @@ struct I8Params {
   int slice_len;     // samples per slice (multiple of 256 when n_slices > 1)
   int n_items;       // n_groups * n_kinds * n_slices
   int rot;           // per-round rotation of the CTA -> item map (spreads the kinds over the CTAs)
+  int dq[2], dr[2];  // (grid + rot) and rot, each split as quotient / remainder by n_kinds (host-computed)
   int diag;          // item kind
   int n_panels;      // diag: total panels along the chan*input axis; slab: panels per channel
   // ---- problem ----
@@ -52,7 +55,7 @@ struct I8Params {
   int probe;         // diagnostics only (corr_set_probe)
   long long n_baselines;
   int2 *vis;
-  unsigned int kinds[kMaxKinds];  // slab: I | J0 << 8 | nblk << 16
+  unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11
 };
 
 struct I8Item {
@@ -67,14 +70,39 @@ struct I8Item {
   int chan, I, J0;   // slab: channel, row panel, first column panel; diag: first panel in J0
 };
 
-// Uniform decode of global item index g (all inputs are kernel parameters / loop counters).
-__device__ __forceinline__ I8Item decode_item(const I8Params &p, int g) {
+// Position of a CTA in the schedule: item g = (s * n_groups + grp) * n_kinds + k, walked WITHOUT
+// divisions (additions, compares and constant-bank reads only), so that ptxas keeps the whole walk
+// and everything decoded from it in uniform registers.  Round r of CTA b takes item
+// r * grid + (b + r * rot) mod grid.
+struct I8Iter {
+  int s, grp, k, b;
+};
+__device__ __forceinline__ void iter_carry(const I8Params &p, I8Iter &c) {
+  if (c.k >= p.n_kinds) { c.k -= p.n_kinds; ++c.grp; }
+  while (c.grp >= p.n_groups) { c.grp -= p.n_groups; ++c.s; }
+}
+__device__ __forceinline__ I8Iter iter_init(const I8Params &p) {
+  I8Iter c;
+  c.b = blockIdx.x;
+  c.s = 0; c.grp = 0; c.k = blockIdx.x;
+  while (c.k >= p.n_kinds) { c.k -= p.n_kinds; ++c.grp; }
+  iter_carry(p, c);
+  return c;
+}
+__device__ __forceinline__ void iter_next(const I8Params &p, I8Iter &c) {
+  c.b += p.rot;
+  int w = 0;
+  if (c.b >= static_cast<int>(gridDim.x)) { c.b -= gridDim.x; w = 1; }  // wrapped: g advances by rot only
+  c.k += p.dr[w];
+  c.grp += p.dq[w];
+  iter_carry(p, c);
+}
+__device__ __forceinline__ bool iter_valid(const I8Params &p, const I8Iter &c) { return c.s < p.n_slices; }
+
+// Decode of a schedule position (all inputs are kernel parameters / uniform counters).
+__device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c) {
   I8Item it;
-  const int per_slice = p.n_groups * p.n_kinds;
-  const int s = g / per_slice;
-  const int rem = g - s * per_slice;
-  const int grp = rem / p.n_kinds;
-  const int k = rem - grp * p.n_kinds;
+  const int s = c.s, grp = c.grp, k = c.k;
   it.t0 = s * p.slice_len;
   it.t1 = min(p.n_time, it.t0 + p.slice_len);
   const int row = 2 * p.n_inputs;  // bytes per (t, c)
@@ -89,7 +117,7 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, int g) {
     it.xa = 0; it.za = 0;
   } else {
     const unsigned kd = p.kinds[k];
-    it.I = kd & 0xFF; it.J0 = (kd >> 8) & 0xFF; it.nblk = (kd >> 16) & 0xFF;
+    it.I = kd & 63; it.J0 = ((kd >> 6) & 31) * 2; it.nblk = ((kd >> 11) & 1) + 1;
     it.chan = grp;
     const bool a_in_b = it.I < it.J0 + it.nblk;
     it.n_load = it.nblk + (a_in_b ? 0 : 1);
@@ -102,14 +130,6 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, int g) {
   else if (it.n_load == 2) { it.bk = 128; it.map = 1; }
   else                     { it.bk = 64;  it.map = 2; }
   return it;
-}
-
-// CTA -> item of round r: round-robin with a per-round rotation (balances kinds of unequal cost).
-__device__ __forceinline__ int item_of_round(const I8Params &p, int r) {
-  const int G = gridDim.x;
-  int b = blockIdx.x + r * p.rot;
-  b -= (b / G) * G;
-  return r * G + b;
 }
 
 template <bool kAtomic>

@@ -1,0 +1,129 @@
+// xengine_i8_epilogue.cuh -- step a3: fold the real Gram blocks in TMEM into packed complex
+// visibilities (included from xengine_i8_kernel.cuh).
+//
+// One epilogue warp owns 32 TMEM lanes = 16 inputs i (lane 2r holds the Re row of input r, lane
+// 2r+1 the Im row).  Per half block (64 TMEM columns = 32 inputs j):
+//   tcgen05.ld 32 columns -> one shfl.xor 1 per column pair gives Re V_ij on the even lane and
+//   Im V_ij on the odd lane  ->  staged in shared memory as [16 rows][32 complex] (row stride
+//   264 B: bank-conflict free for both directions)  ->  read back one ROW per instruction, so a
+//   warp store covers 256 contiguous bytes of the packed triangle (the direct lane->global
+//   mapping touched 32 different sectors per store and was store-sector bound).
+#pragma once
+
+namespace corr {
+
+constexpr int kEpiRowBytes = 272;  // 32 complex int32 + one alignment slot, 16-byte multiple
+constexpr int kEpiWarpBytes = 16 * kEpiRowBytes;  // 4224 B per epilogue warp
+
+__device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_base, uint8_t *stage_buf,
+                                            uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
+                                            int hsel, int lane) {
+  const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
+  const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
+  const bool atomic = p.n_slices > 1;
+  int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kEpiRowBytes / 4) + part;
+  uint32_t ring = 0;
+  I8Iter cur = iter_init(p);
+  for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
+    if (!iter_valid(p, cur)) continue;
+    const I8Item it = decode_item(p, cur);
+    const int n_chunks = (it.nblk + 1) >> 1;
+    for (int q = 0; q < n_chunks; ++q) {
+      const uint32_t e = ring + q;
+      mbar_wait(&acc_full[e & 1], (e >> 1) & 1);
+      tc_fence_after();
+      const uint32_t tchunk = tmem_base + (static_cast<uint32_t>(ew * 32) << 16) + (e & 1) * kAccCols;
+      const int nb_here = min(2, it.nblk - 2 * q);
+      for (int bb = 0; bb < nb_here; ++bb) {
+        const int b = 2 * q + bb;
+        // what this warp's 16 rows and the block's 64 column-inputs are (all warp-uniform)
+        int chan_w, i0_w, j_blk0;
+        bool diag_blk;
+        if (p.diag) {
+          const int panel = it.J0 + b;
+          chan_w = p.pair_mode ? 2 * panel + (ew >> 1) : panel;
+          i0_w = p.pair_mode ? (ew & 1) * 16 : ew * 16;
+          j_blk0 = 0;
+          diag_blk = true;
+        } else {
+          chan_w = it.chan;
+          i0_w = it.I * 64 + ew * 16;
+          j_blk0 = (it.J0 + b) * 64;
+          diag_blk = (it.J0 + b) == it.I;
+        }
+        const bool warp_ok = (chan_w < p.n_chan) && (i0_w < p.n_inputs);
+        // this lane pair's row: input i_row, its first packed element and how many columns it keeps
+        const int i_row = i0_w + rl;
+        const long long e_row = static_cast<long long>(chan_w) * p.n_baselines + i_row * (i_row + 1) / 2;
+        {
+          const int h = hsel;
+          int j0;
+          bool ok;
+          if (p.pair_mode) { j0 = 0; ok = (h == (ew >> 1)); }
+          else { j0 = j_blk0 + h * 32; ok = (j0 < p.n_inputs) && (!diag_blk || h * 32 <= ew * 16 + 15); }
+          if (!(ok && warp_ok)) continue;  // above the diagonal / other channel / past N_I (next block)
+          // row r of the staging buffer starts on a 16-byte boundary; its elements are shifted by one
+          // slot when the row's first packed element has an odd index, so that 16-byte aligned pairs in
+          // global memory are 16-byte aligned in shared memory too (bulk copies need both).
+          const int par = static_cast<int>((e_row + j0) & 1);
+          int *st_row = st_w + par * 2;
+          uint32_t v[32];
+          tmem_ld_32x32(tchunk + bb * 128 + h * 64, v);
+          // the previous half block's bulk stores must have read the staging buffer before it is reused
+          if (lane < 16) bulk_wait_read_all();
+          __syncwarp();
+#pragma unroll
+          for (int cb = 0; cb < 2; ++cb) {
+            if (cb == 1) tmem_ld_32x32(tchunk + bb * 128 + h * 64 + 32, v);
+            tmem_ld_wait();
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) {
+              const int other = __shfl_xor_sync(0xffffffffu, static_cast<int>(v[2 * jj + 1]), 1);
+              int val = part ? (static_cast<int>(v[2 * jj]) - other) : (static_cast<int>(v[2 * jj]) + other);
+              if (part && (j0 + cb * 16 + jj) == i_row) val = 0;  // Im of an autocorrelation is exactly 0
+              st_row[(cb * 16 + jj) * 2] = val;                   // even lane: Re -> .x, odd lane: Im -> .y
+            }
+          }
+          fence_proxy_async();  // make the generic-proxy writes visible to the bulk-copy (async) proxy
+          __syncwarp();
+          if (lane < 16 && !(p.probe & 16)) {
+            // lane r ships row r: elements j0 .. j0+cnt-1 of input i = i0_w + r
+            const int i = i0_w + lane;
+            const int cnt = (i < p.n_inputs) ? min(32, min(i, p.n_inputs - 1) - j0 + 1) : 0;
+            if (cnt > 0) {
+              const long long e0 = static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j0;
+              const int sh = static_cast<int>(e0 & 1);
+              const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kEpiRowBytes) + sh;  // element 0
+              int2 *grow = p.vis + e0;
+              int head = sh;                         // one leading element if e0 is odd
+              int body = (cnt - head) & ~1;          // aligned pairs
+              if (cnt < head) { head = cnt; body = 0; }
+              const int tail = cnt - head - body;    // one trailing element
+              if (head) {
+                const int2 x = srow[0];
+                if (atomic) put_vis<true>(grow, x.x, x.y); else put_vis<false>(grow, x.x, x.y);
+              }
+              if (body) {
+                if (atomic) bulk_reduce_add_s32(grow + head, srow + head, body * 8);
+                else        bulk_store(grow + head, srow + head, body * 8);
+              }
+              if (tail) {
+                const int2 x = srow[cnt - 1];
+                if (atomic) put_vis<true>(grow + cnt - 1, x.x, x.y); else put_vis<false>(grow + cnt - 1, x.x, x.y);
+              }
+            }
+            bulk_commit();
+          }
+        }
+      }
+      // every tcgen05.ld of this ring entry has completed (wait::ld above): hand it back
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_empty[e & 1]);
+    }
+    ring += n_chunks;
+  }
+  if (lane < 16) bulk_wait_all();  // all visibilities written before the CTA retires
+}
+
+}  // namespace corr
