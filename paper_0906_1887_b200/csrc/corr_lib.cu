@@ -135,10 +135,12 @@ void plan_i8(corr_handle *h) {
   }
   ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices;
   ip.rot = ip.n_kinds > 1 ? 1 : 0;
-  ip.stage_bytes = 4 * 64 * 128;  // 32 KB: 1 x 256, 2 x 128 or 3-4 x 64 time rows of 128 B
+  // 32 KB stages: 1 x 256, 2 x 128 or 4 x 64 time rows of 128 B; 48 KB when items fetch 3 panels (3 x 128)
+  ip.stage_bytes = (!ip.diag && max_load == 3) ? 3 * 128 * 128 : 4 * 64 * 128;
   const int epi_bytes = corr::kEpiWarps * corr::kEpiWarpBytes;  // epilogue staging behind the stage ring
-  ip.stages = std::min<int>(corr::kMaxStages, (232448 - 4096 - epi_bytes) / ip.stage_bytes);
-  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + epi_bytes + 1024;
+  const int bar_bytes = 256;  // 2 * kMaxStages + 4 mbarriers and the TMEM base address
+  ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ip.stage_bytes);
+  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + epi_bytes + bar_bytes;
   h->grid_i8 = std::min(ip.n_items, h->n_sms);
   const int deltas[2] = {h->grid_i8 + ip.rot, ip.rot};
   for (int w = 0; w < 2; ++w) { ip.dq[w] = deltas[w] / ip.n_kinds; ip.dr[w] = deltas[w] % ip.n_kinds; }

@@ -128,6 +128,7 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
   }
   if (it.n_load == 1)      { it.bk = 256; it.map = 0; }
   else if (it.n_load == 2) { it.bk = 128; it.map = 1; }
+  else if (it.n_load == 3 && p.stage_bytes >= 3 * 128 * kPanelBytes) { it.bk = 128; it.map = 1; }
   else                     { it.bk = 64;  it.map = 2; }
   return it;
 }

@@ -28,13 +28,15 @@ __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_
 __global__ void __launch_bounds__(kI8Threads, 1)
 xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
                   const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  __shared__ __align__(8) uint64_t full_bar[kMaxStages];
-  __shared__ __align__(8) uint64_t empty_bar[kMaxStages];
-  __shared__ __align__(8) uint64_t acc_full[2];
-  __shared__ __align__(8) uint64_t acc_empty[2];
-  __shared__ uint32_t tmem_base_smem;
+  // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
+  // 128-byte swizzle needs: [stage ring][epilogue staging][mbarriers + TMEM base].
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(p.stages) * p.stage_bytes +
+                                                    kEpiWarps * kEpiWarpBytes);
+  uint64_t *empty_bar = full_bar + kMaxStages;
+  uint64_t *acc_full = empty_bar + kMaxStages;
+  uint64_t *acc_empty = acc_full + 2;
+  uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(acc_empty + 2);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
