@@ -10,6 +10,7 @@
 #include <chrono>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <queue>
 #include <vector>
@@ -69,7 +70,7 @@ struct corr_handle {
   int turn_mode;
   int probe;
   // CI8 plan
-  int pair_mode, grid_i8;
+  int pair_mode, grid_i8, use_pairs;
   size_t smem_i8;
   corr::I8Params ip;  // schedule + problem, passed by value into the constant bank at each launch
   void *d_scratch;  // corner-turn output (standalone mode)
@@ -123,12 +124,21 @@ void plan_i8(corr_handle *h) {
     ip.n_panels = panels_per_chan;
     ip.n_groups = C;
     int k = 0;
-    for (int I = panels_per_chan - 1; I >= 0; --I)
-      for (int J0 = 0; J0 <= I; J0 += 2) {
-        const int nblk = std::min(2, I - J0 + 1);
-        max_load = std::max(max_load, (I < J0 + nblk) ? nblk : nblk + 1);
-        ip.kinds[k++] = static_cast<unsigned short>(I | ((J0 >> 1) << 6) | ((nblk - 1) << 11));
-      }
+    if (h->use_pairs) {
+      // CTA pairs: 256 x 256 tiles (row-panel pair Ip, column-panel pair Jp <= Ip)
+      ip.pair2 = 1;
+      const int pp = (panels_per_chan + 1) / 2;
+      for (int Ip = pp - 1; Ip >= 0; --Ip)
+        for (int Jp = 0; Jp <= Ip; ++Jp) ip.kinds[k++] = static_cast<unsigned short>(Ip | (Jp << 6));
+      max_load = 2;
+    } else {
+      for (int I = panels_per_chan - 1; I >= 0; --I)
+        for (int J0 = 0; J0 <= I; J0 += 2) {
+          const int nblk = std::min(2, I - J0 + 1);
+          max_load = std::max(max_load, (I < J0 + nblk) ? nblk : nblk + 1);
+          ip.kinds[k++] = static_cast<unsigned short>(I | ((J0 >> 1) << 6) | ((nblk - 1) << 11));
+        }
+    }
     ip.n_kinds = k;
     ip.n_slices = 1;
     ip.slice_len = T;
@@ -141,8 +151,9 @@ void plan_i8(corr_handle *h) {
   const int bar_bytes = 256;  // 2 * kMaxStages + 4 mbarriers and the TMEM base address
   ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ip.stage_bytes);
   h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + epi_bytes + bar_bytes;
-  h->grid_i8 = std::min(ip.n_items, h->n_sms);
-  const int deltas[2] = {h->grid_i8 + ip.rot, ip.rot};
+  ip.units = std::min(ip.n_items, ip.pair2 ? h->n_sms / 2 : h->n_sms);
+  h->grid_i8 = ip.pair2 ? 2 * ip.units : ip.units;
+  const int deltas[2] = {ip.units + ip.rot, ip.rot};
   for (int w = 0; w < 2; ++w) { ip.dq[w] = deltas[w] / ip.n_kinds; ip.dr[w] = deltas[w] % ip.n_kinds; }
 }
 
@@ -262,8 +273,11 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
 
   cudaError_t e = cudaSuccess;
   if (dtype == CORR_CI8) {
+    h->use_pairs = getenv("CORR_NO_PAIRS") ? 0 : 1;  // CTA pairs (cta_group::2) for N_I >= 128
     plan_i8(h);
     e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(corr::xengine_i8_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
   } else {
     std::vector<int2> items;
     plan_f32(h, items);
@@ -425,7 +439,8 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.vis = static_cast<int2 *>(d_vis);
   ip.probe = h->probe;
   if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
-  corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+  if (ip.pair2) corr::xengine_i8_pair_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+  else          corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }

@@ -46,6 +46,8 @@ struct I8Params {
   int rot;           // per-round rotation of the CTA -> item map (spreads the kinds over the CTAs)
   int dq[2], dr[2];  // (grid + rot) and rot, each split as quotient / remainder by n_kinds (host-computed)
   int diag;          // item kind
+  int pair2;         // 1: CTA pairs (cta_group::2): an item is a 256 x 256 tile, 128 rows per CTA
+  int units;         // schedule walkers: CTAs, or CTA pairs when pair2
   int n_panels;      // diag: total panels along the chan*input axis; slab: panels per channel
   // ---- problem ----
   int n_time, n_inputs, n_chan;
@@ -61,6 +63,7 @@ struct I8Params {
 struct I8Item {
   int t0, t1;        // time slice
   int nblk;          // 128-column blocks (1..4)
+  int nblk_load;     // B panels this CTA fetches (= nblk, except 1 in pair mode)
   int n_load;        // panels fetched per k-step (nblk, +1 when A is not one of the B panels)
   int a_slot;        // slab: smem slot of the A panel; diag: unused (A = B = slot b)
   int x0, z0;        // TMA coordinates of block 0 (block b at x0 + b*dx, z0 + b*dz)
@@ -83,8 +86,8 @@ __device__ __forceinline__ void iter_carry(const I8Params &p, I8Iter &c) {
 }
 __device__ __forceinline__ I8Iter iter_init(const I8Params &p) {
   I8Iter c;
-  c.b = blockIdx.x;
-  c.s = 0; c.grp = 0; c.k = blockIdx.x;
+  c.b = static_cast<int>(blockIdx.x) >> p.pair2;
+  c.s = 0; c.grp = 0; c.k = c.b;
   while (c.k >= p.n_kinds) { c.k -= p.n_kinds; ++c.grp; }
   iter_carry(p, c);
   return c;
@@ -92,7 +95,7 @@ __device__ __forceinline__ I8Iter iter_init(const I8Params &p) {
 __device__ __forceinline__ void iter_next(const I8Params &p, I8Iter &c) {
   c.b += p.rot;
   int w = 0;
-  if (c.b >= static_cast<int>(gridDim.x)) { c.b -= gridDim.x; w = 1; }  // wrapped: g advances by rot only
+  if (c.b >= p.units) { c.b -= p.units; w = 1; }  // wrapped: g advances by rot only
   c.k += p.dr[w];
   c.grp += p.dq[w];
   iter_carry(p, c);
@@ -100,7 +103,7 @@ __device__ __forceinline__ void iter_next(const I8Params &p, I8Iter &c) {
 __device__ __forceinline__ bool iter_valid(const I8Params &p, const I8Iter &c) { return c.s < p.n_slices; }
 
 // Decode of a schedule position (all inputs are kernel parameters / uniform counters).
-__device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c) {
+__device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c, int rank = 0) {
   I8Item it;
   const int s = c.s, grp = c.grp, k = c.k;
   it.t0 = s * p.slice_len;
@@ -115,6 +118,19 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
     if (p.turned) { it.x0 = 0; it.z0 = panel0; it.dx = 0; it.dz = 1; }
     else          { it.x0 = panel0 * kPanelBytes; it.z0 = 0; it.dx = kPanelBytes; it.dz = 0; }
     it.xa = 0; it.za = 0;
+  } else if (p.pair2) {
+    // CTA `rank` of the pair owns row panel 2*Ip + rank and fetches column panel 2*Jp + rank (its half of B)
+    const unsigned kd = p.kinds[k];
+    const int Ip = kd & 63, Jp = (kd >> 6) & 31;
+    it.I = 2 * Ip + rank; it.J0 = 2 * Jp; it.nblk = 2;
+    it.chan = grp;
+    const bool same = (Ip == Jp);  // diagonal tile: the CTA's A panel is its B half
+    it.n_load = same ? 1 : 2;
+    it.a_slot = same ? 0 : 1;
+    const int xc = p.turned ? 0 : grp * row;
+    it.x0 = xc + (it.J0 + rank) * kPanelBytes; it.z0 = p.turned ? grp : 0; it.dx = 0; it.dz = 0;
+    it.xa = xc + it.I * kPanelBytes; it.za = it.z0;
+    it.nblk_load = 1;
   } else {
     const unsigned kd = p.kinds[k];
     it.I = kd & 63; it.J0 = ((kd >> 6) & 31) * 2; it.nblk = ((kd >> 11) & 1) + 1;
@@ -126,6 +142,7 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
     it.x0 = xc + it.J0 * kPanelBytes; it.z0 = p.turned ? grp : 0; it.dx = kPanelBytes; it.dz = 0;
     it.xa = xc + it.I * kPanelBytes; it.za = it.z0;
   }
+  if (!p.pair2) it.nblk_load = it.nblk;
   if (it.n_load == 1)      { it.bk = 256; it.map = 0; }
   else if (it.n_load == 2) { it.bk = 128; it.map = 1; }
   else if (it.n_load == 3 && p.stage_bytes >= 3 * 128 * kPanelBytes) { it.bk = 128; it.map = 1; }

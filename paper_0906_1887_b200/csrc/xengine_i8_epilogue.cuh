@@ -17,7 +17,7 @@ constexpr int kEpiWarpBytes = 16 * kEpiRowBytes;  // 4224 B per epilogue warp
 
 __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_base, uint8_t *stage_buf,
                                             uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
-                                            int hsel, int lane) {
+                                            int hsel, int lane, int rank, bool pair) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
   const bool atomic = p.n_slices > 1;
@@ -26,7 +26,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
   I8Iter cur = iter_init(p);
   for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
     if (!iter_valid(p, cur)) continue;
-    const I8Item it = decode_item(p, cur);
+    const I8Item it = decode_item(p, cur, rank);
     const int n_chunks = (it.nblk + 1) >> 1;
     for (int q = 0; q < n_chunks; ++q) {
       const uint32_t e = ring + q;
@@ -36,6 +36,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
       const int nb_here = min(2, it.nblk - 2 * q);
       for (int bb = 0; bb < nb_here; ++bb) {
         const int b = 2 * q + bb;
+        if (!p.diag && it.J0 + b > it.I) continue;  // block above the diagonal (pair tiles on the diagonal)
         // what this warp's 16 rows and the block's 64 column-inputs are (all warp-uniform)
         int chan_w, i0_w, j_blk0;
         bool diag_blk;
@@ -119,7 +120,10 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
       // every tcgen05.ld of this ring entry has completed (wait::ld above): hand it back
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&acc_empty[e & 1]);
+      if (lane == 0) {
+        if (pair) mbar_arrive_cluster(mapa_u32(&acc_empty[e & 1], 0));  // the leader's MMA thread owns the wait
+        else      mbar_arrive(&acc_empty[e & 1]);
+      }
     }
     ring += n_chunks;
   }

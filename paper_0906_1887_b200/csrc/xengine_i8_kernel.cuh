@@ -6,28 +6,31 @@ namespace corr {
 
 // NK back-to-back MMAs over the NK k-steps (32 time samples = 4096 B of a panel each) of one stage.
 // Straight-line code: the descriptor words of all NK issues are independent of one another.
-template <int NK>
+template <int NK, bool kPair>
 __device__ __forceinline__ void issue_k(uint32_t d, uint32_t lo_a, uint32_t lo_b, uint32_t hi, uint32_t idesc,
                                         uint32_t acc0) {
 #pragma unroll
   for (int k = 0; k < NK; ++k) {
     const uint64_t da = (static_cast<uint64_t>(hi) << 32) | (lo_a + k * (32 * kPanelBytes / 16));
     const uint64_t db = (static_cast<uint64_t>(hi) << 32) | (lo_b + k * (32 * kPanelBytes / 16));
-    mma_i8_ss(d, da, db, idesc, k == 0 ? acc0 : 1u);
+    if (kPair) mma_i8_ss_2sm(d, da, db, idesc, k == 0 ? acc0 : 1u);
+    else       mma_i8_ss(d, da, db, idesc, k == 0 ? acc0 : 1u);
   }
 }
+template <bool kPair>
 __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_b, uint32_t hi, uint32_t idesc,
                                          uint32_t acc0, int nk) {
   for (int k = 0; k < nk; ++k) {
     const uint64_t da = (static_cast<uint64_t>(hi) << 32) | (lo_a + k * (32 * kPanelBytes / 16));
     const uint64_t db = (static_cast<uint64_t>(hi) << 32) | (lo_b + k * (32 * kPanelBytes / 16));
-    mma_i8_ss(d, da, db, idesc, k == 0 ? acc0 : 1u);
+    if (kPair) mma_i8_ss_2sm(d, da, db, idesc, k == 0 ? acc0 : 1u);
+    else       mma_i8_ss(d, da, db, idesc, k == 0 ? acc0 : 1u);
   }
 }
 
-__global__ void __launch_bounds__(kI8Threads, 1)
-xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
-                  const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
+template <bool kPair>
+__device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, const CUtensorMap &tmap128,
+                                                const CUtensorMap &tmap64, const I8Params &p) {
   // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
   // 128-byte swizzle needs: [stage ring][epilogue staging][mbarriers + TMEM base].
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -40,7 +43,8 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
-  const int n_rounds = (p.n_items + gridDim.x - 1) / gridDim.x;
+  const int n_rounds = (p.n_items + p.units - 1) / p.units;
+  const int rank = kPair ? static_cast<int>(cluster_ctarank()) : 0;  // CTA within the pair; 0 issues the MMAs
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmap256);
@@ -52,13 +56,13 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
     }
     for (int r = 0; r < 2; ++r) {
       mbar_init(&acc_full[r], 1);
-      mbar_init(&acc_empty[r], kEpiWarps);  // one arrive per epilogue warp
+      mbar_init(&acc_empty[r], kEpiWarps * (kPair ? 2 : 1));  // one arrive per epilogue warp (of both CTAs)
     }
     fence_mbar_init();
   }
-  if (warp == 2) tmem_alloc(&tmem_base_smem, 512);
+  if (warp == 2) { if (kPair) tmem_alloc_2sm(&tmem_base_smem, 512); else tmem_alloc(&tmem_base_smem, 512); }
   tc_fence_before();
-  __syncthreads();
+  if (kPair) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
@@ -66,27 +70,35 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
     // ===================================================================== TMA producer
     if (lane == 0 && !(p.probe & 8)) {
       const uint64_t pol = policy_evict_normal();
+      const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
       uint32_t phase = 0;
       I8Iter cur = iter_init(p);
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
-        const I8Item it = decode_item(p, cur);
+        const I8Item it = decode_item(p, cur, rank);
         const CUtensorMap *map = it.map == 0 ? &tmap256 : (it.map == 1 ? &tmap128 : &tmap64);
         const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
         for (int t = it.t0; t < it.t1; t += it.bk) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           if (p.probe & 2) {
-            mbar_arrive(&full_bar[stage]);
+            if (rank == 0) mbar_arrive(&full_bar[stage]);
           } else {
-            mbar_expect_tx(&full_bar[stage], panel_bytes * it.n_load);
+            // pair mode: both CTAs' boxes complete on the LEADER's barrier, which expects the bytes of both
+            if (rank == 0) mbar_expect_tx(&full_bar[stage], panel_bytes * it.n_load * (kPair ? 2 : 1));
             uint8_t *dst = smem + static_cast<size_t>(stage) * p.stage_bytes;
+            const uint32_t bar2 = kPair ? full_leader + stage * 8 : 0;
             for (int l = 0; l < it.n_load; ++l) {
-              const bool is_a = l >= it.nblk;
+              const bool is_a = l >= it.nblk_load;
               const int x = is_a ? it.xa : it.x0 + l * it.dx;
               const int z = is_a ? it.za : it.z0 + l * it.dz;
-              if (p.turned) tma_load_3d(dst + l * panel_bytes, map, &full_bar[stage], x, t, z, pol);
-              else          tma_load_2d(dst + l * panel_bytes, map, &full_bar[stage], x, t, pol);
+              if (kPair) {
+                if (p.turned) tma_load_3d_2sm(dst + l * panel_bytes, map, bar2, x, t, z, pol);
+                else          tma_load_2d_2sm(dst + l * panel_bytes, map, bar2, x, t, pol);
+              } else {
+                if (p.turned) tma_load_3d(dst + l * panel_bytes, map, &full_bar[stage], x, t, z, pol);
+                else          tma_load_2d(dst + l * panel_bytes, map, &full_bar[stage], x, t, pol);
+              }
             }
           }
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
@@ -98,19 +110,20 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
     // The whole warp walks the (uniform) schedule so that loop state lives in uniform registers;
     // one lane issues.  Descriptor low words are advanced by plain adds (all offsets are multiples
     // of 16 B and the address field cannot carry into the LBO field below 256 KB).
-    if (lane == 0) {
+    if (lane == 0 && rank == 0) {
       constexpr bool leader = true;
       int stage = 0;
       uint32_t phase = 0;
       uint32_t ring = 0;  // accumulator ring entries handed out so far
-      constexpr uint32_t kIdesc128 = idesc_i8_mn(128, 128), kIdesc256 = idesc_i8_mn(128, 256);
+      constexpr uint32_t kIdesc128 = idesc_i8_mn(128, 128);
+      constexpr uint32_t kIdesc256 = kPair ? idesc_i8_mn(256, 256) : idesc_i8_mn(128, 256);
       constexpr uint32_t kDescHi = static_cast<uint32_t>(((1024ull >> 4) | (1ull << 14) | (2ull << 29)));
       const uint32_t smem_lo = (smem_u32(smem) & 0x3FFFFu) >> 4;
       const uint32_t tmem_u = tmem_base;
       I8Iter cur = iter_init(p);
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
-        const I8Item it = decode_item(p, cur);
+        const I8Item it = decode_item(p, cur, 0);
         // decode_item divides, so its results sit in vector registers; one REDUX each brings what the
         // issue loop needs into uniform registers (an R2UR in front of every MMA costs ~60 cycles).
         const int u_bk = it.bk;
@@ -138,22 +151,26 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
               for (int b = 0; b < u_nblk; ++b) {
                 const uint32_t dcol = ((b & 2) ? d1 : d0) + (b & 1) * 128;
                 const uint32_t lo_b = lo_stage + b * panel16;
-                if (nk == 2)      issue_k<2>(dcol, lo_b, lo_b, kDescHi, kIdesc128, acc0);
-                else              issue_kn(dcol, lo_b, lo_b, kDescHi, kIdesc128, acc0, nk);
+                if (nk == 2)      issue_k<2, false>(dcol, lo_b, lo_b, kDescHi, kIdesc128, acc0);
+                else              issue_kn<false>(dcol, lo_b, lo_b, kDescHi, kIdesc128, acc0, nk);
               }
             } else {
               const uint32_t lo_a = lo_stage + a_off;
-              if (nk == 2)      issue_k<2>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
-              else if (nk == 4) issue_k<4>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
-              else if (nk == 8) issue_k<8>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
-              else              issue_kn(d0, lo_a, lo_stage, kDescHi, idesc0, acc0, nk);
+              if (nk == 2)      issue_k<2, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
+              else if (nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
+              else if (nk == 8) issue_k<8, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
+              else              issue_kn<kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0, nk);
             }
           }
-          if (leader && !(p.probe & 8)) mma_commit(&empty_bar[stage]);  // frees the stage when these MMAs retire
+          if (leader && !(p.probe & 8)) {  // frees the stage (in both CTAs of a pair) when these MMAs retire
+            if (kPair) mma_commit_2sm(&empty_bar[stage], 3); else mma_commit(&empty_bar[stage]);
+          }
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
         }
         if (leader)
-          for (int q = 0; q < n_chunks; ++q) mma_commit(&acc_full[(ring + q) & 1]);
+          for (int q = 0; q < n_chunks; ++q) {
+            if (kPair) mma_commit_2sm(&acc_full[(ring + q) & 1], 3); else mma_commit(&acc_full[(ring + q) & 1]);
+          }
         ring += n_chunks;
       }
     }
@@ -162,15 +179,28 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
     const int ew = (warp - 4) & 3;   // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = (warp - 4) >> 2;  // which half (64 TMEM columns) of every block this warp folds
     i8_epilogue(p, tmem_base, smem + static_cast<size_t>(p.stages) * p.stage_bytes + (warp - 4) * kEpiWarpBytes,
-                acc_full, acc_empty, n_rounds, ew, hsel, lane);
+                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair);
   }
 
   tc_fence_before();
-  __syncthreads();
+  if (kPair) cluster_sync_all(); else __syncthreads();
   if (warp == 2) {
     tc_fence_after();
-    tmem_dealloc(tmem_base, 512);
+    if (kPair) tmem_dealloc_2sm(tmem_base, 512); else tmem_dealloc(tmem_base, 512);
   }
+}
+
+__global__ void __launch_bounds__(kI8Threads, 1)
+xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
+                  const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
+  xengine_i8_body<false>(tmap256, tmap128, tmap64, p);
+}
+
+// CTA pairs: tcgen05.mma.cta_group::2, M = 256 (one 128-row panel per CTA), each CTA stages half of B.
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kI8Threads, 1)
+xengine_i8_pair_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
+                       const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
+  xengine_i8_body<true>(tmap256, tmap128, tmap64, p);
 }
 
 }  // namespace corr
