@@ -124,7 +124,7 @@ void plan_i8(corr_handle *h) {
     ip.n_panels = panels_per_chan;
     ip.n_groups = C;
     int k = 0;
-    if (h->use_pairs) {
+    if (h->use_pairs && panels_per_chan >= 8) {  // measured: pairs win from N_I = 512 up (c3, P = 4, loses 25 %)
       // CTA pairs: 256 x 256 tiles (row-panel pair Ip, column-panel pair Jp <= Ip)
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;

@@ -2,12 +2,15 @@
 // visibilities (included from xengine_i8_kernel.cuh).
 //
 // One epilogue warp owns 32 TMEM lanes = 16 inputs i (lane 2r holds the Re row of input r, lane
-// 2r+1 the Im row).  Per half block (64 TMEM columns = 32 inputs j):
+// 2r+1 the Im row) and one half (64 TMEM columns = 32 inputs j) of every block:
 //   tcgen05.ld 32 columns -> one shfl.xor 1 per column pair gives Re V_ij on the even lane and
-//   Im V_ij on the odd lane  ->  staged in shared memory as [16 rows][32 complex] (row stride
-//   264 B: bank-conflict free for both directions)  ->  read back one ROW per instruction, so a
-//   warp store covers 256 contiguous bytes of the packed triangle (the direct lane->global
-//   mapping touched 32 different sectors per store and was store-sector bound).
+//   Im V_ij on the odd lane -> staged in shared memory as [16 rows][32 complex] (row stride 272 B)
+//   -> shipped one packed-triangle ROW at a time:
+//        whole integrations : 32 lanes x 8 B = 256 contiguous bytes per store instruction;
+//        time-sliced items  : one cp.reduce.async.bulk.add.s32 per row (integer reduce-add in L2)
+//                             for the 16-byte aligned body + <= 2 scalar atomics for the edges.
+// The TMEM buffer is handed back with a RELAXED mbarrier arrive: a releasing arrive made the warp
+// wait (MEMBAR) for all of its visibility stores to land, which serialised epilogue and DRAM writes.
 #pragma once
 
 namespace corr {
@@ -55,7 +58,6 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
         const bool warp_ok = (chan_w < p.n_chan) && (i0_w < p.n_inputs);
         // this lane pair's row: input i_row, its first packed element and how many columns it keeps
         const int i_row = i0_w + rl;
-        const long long e_row = static_cast<long long>(chan_w) * p.n_baselines + i_row * (i_row + 1) / 2;
         {
           const int h = hsel;
           int j0;
@@ -63,15 +65,15 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
           if (p.pair_mode) { j0 = 0; ok = (h == (ew >> 1)); }
           else { j0 = j_blk0 + h * 32; ok = (j0 < p.n_inputs) && (!diag_blk || h * 32 <= ew * 16 + 15); }
           if (!(ok && warp_ok)) continue;  // above the diagonal / other channel / past N_I (next block)
-          // row r of the staging buffer starts on a 16-byte boundary; its elements are shifted by one
-          // slot when the row's first packed element has an odd index, so that 16-byte aligned pairs in
-          // global memory are 16-byte aligned in shared memory too (bulk copies need both).
-          const int par = static_cast<int>((e_row + j0) & 1);
+          // sliced (accumulating) items ship rows with bulk reduce-add: 16-byte aligned pairs in global memory must
+          // be 16-byte aligned in shared memory too, so a row is shifted by one slot when its first element is odd
+          const int par = atomic ? static_cast<int>((static_cast<long long>(chan_w) * p.n_baselines +
+                                                      i_row * (i_row + 1) / 2 + j0) & 1) : 0;
           int *st_row = st_w + par * 2;
           uint32_t v[32];
           tmem_ld_32x32(tchunk + bb * 128 + h * 64, v);
           // the previous half block's bulk stores must have read the staging buffer before it is reused
-          if (lane < 16) bulk_wait_read_all();
+          if (atomic && lane < 16) bulk_wait_read_all();  // earlier bulk reduces have read the staging buffer
           __syncwarp();
 #pragma unroll
           for (int cb = 0; cb < 2; ++cb) {
@@ -85,36 +87,57 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
               st_row[(cb * 16 + jj) * 2] = val;                   // even lane: Re -> .x, odd lane: Im -> .y
             }
           }
-          fence_proxy_async();  // make the generic-proxy writes visible to the bulk-copy (async) proxy
+          if (atomic) fence_proxy_async();  // generic-proxy writes -> visible to the bulk (async) proxy
           __syncwarp();
-          if (lane < 16 && !(p.probe & 16)) {
-            // lane r ships row r: elements j0 .. j0+cnt-1 of input i = i0_w + r
-            const int i = i0_w + lane;
-            const int cnt = (i < p.n_inputs) ? min(32, min(i, p.n_inputs - 1) - j0 + 1) : 0;
-            if (cnt > 0) {
-              const long long e0 = static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j0;
-              const int sh = static_cast<int>(e0 & 1);
-              const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kEpiRowBytes) + sh;  // element 0
-              int2 *grow = p.vis + e0;
-              int head = sh;                         // one leading element if e0 is odd
-              int body = (cnt - head) & ~1;          // aligned pairs
-              if (cnt < head) { head = cnt; body = 0; }
-              const int tail = cnt - head - body;    // one trailing element
-              if (head) {
-                const int2 x = srow[0];
-                if (atomic) put_vis<true>(grow, x.x, x.y); else put_vis<false>(grow, x.x, x.y);
+          if (atomic) {
+            if (lane < 16 && !(p.probe & 16)) {
+              // lane r ships row r: elements j0 .. j0+cnt-1 of input i = i0_w + r
+              const int i = i0_w + lane;
+              const int cnt = (i < p.n_inputs) ? min(32, min(i, p.n_inputs - 1) - j0 + 1) : 0;
+              if (cnt > 0) {
+                const long long e0 = static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j0;
+                const int sh = static_cast<int>(e0 & 1);
+                const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kEpiRowBytes) + sh;  // element 0
+                int2 *grow = p.vis + e0;
+                int head = sh;                         // one leading element if e0 is odd
+                int body = (cnt - head) & ~1;          // aligned pairs
+                if (cnt < head) { head = cnt; body = 0; }
+                const int tail = cnt - head - body;    // one trailing element
+                if (head) {
+                  const int2 x = srow[0];
+                  if (atomic) put_vis<true>(grow, x.x, x.y); else put_vis<false>(grow, x.x, x.y);
+                }
+                if (body) {
+                  if (atomic) bulk_reduce_add_s32(grow + head, srow + head, body * 8);
+                  else        bulk_store(grow + head, srow + head, body * 8);
+                }
+                if (tail) {
+                  const int2 x = srow[cnt - 1];
+                  if (atomic) put_vis<true>(grow + cnt - 1, x.x, x.y); else put_vis<false>(grow + cnt - 1, x.x, x.y);
+                }
               }
-              if (body) {
-                if (atomic) bulk_reduce_add_s32(grow + head, srow + head, body * 8);
-                else        bulk_store(grow + head, srow + head, body * 8);
-              }
-              if (tail) {
-                const int2 x = srow[cnt - 1];
-                if (atomic) put_vis<true>(grow + cnt - 1, x.x, x.y); else put_vis<false>(grow + cnt - 1, x.x, x.y);
-              }
+              bulk_commit();
             }
-            bulk_commit();
+
+          } else if (!(p.probe & 16)) {
+            // one packed-triangle row per instruction: 32 lanes x 8 B = 256 contiguous bytes
+            const int j = j0 + lane;
+            int i = i0_w;
+            int2 *row = p.vis + (static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j);
+            const int2 *src = reinterpret_cast<const int2 *>(stage_buf) + lane;
+#pragma unroll 4
+            for (int rr = 0; rr < 16; ++rr) {
+              if (i >= p.n_inputs) break;
+              const int2 val = src[rr * (kEpiRowBytes / 8)];
+              if (j <= i && j < p.n_inputs) {
+                if (atomic) put_vis<true>(row, val.x, val.y);
+                else        put_vis<false>(row, val.x, val.y);
+              }
+              ++i;
+              row += i;  // next row of the triangle starts i+1 elements further on
+            }
           }
+          __syncwarp();
         }
       }
       // every tcgen05.ld of this ring entry has completed (wait::ld above): hand it back
@@ -122,12 +145,12 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
       __syncwarp();
       if (lane == 0) {
         if (pair) mbar_arrive_cluster(mapa_u32(&acc_empty[e & 1], 0));  // the leader's MMA thread owns the wait
-        else      mbar_arrive(&acc_empty[e & 1]);
+        else      mbar_arrive_relaxed(&acc_empty[e & 1]);
       }
     }
     ring += n_chunks;
   }
-  if (lane < 16) bulk_wait_all();  // all visibilities written before the CTA retires
+  if (atomic && lane < 16) bulk_wait_all();  // all reduce-adds performed before the CTA retires
 }
 
 }  // namespace corr
