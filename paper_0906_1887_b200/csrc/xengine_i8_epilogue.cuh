@@ -20,7 +20,7 @@ constexpr int kEpiWarpBytes = 16 * kEpiRowBytes;  // 4224 B per epilogue warp
 
 __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_base, uint8_t *stage_buf,
                                             uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
-                                            int hsel, int lane, int rank, bool pair) {
+                                            int hsel, int lane, int rank, bool pair, int probe) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
   const bool atomic = p.n_slices > 1;
@@ -90,7 +90,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
           if (atomic) fence_proxy_async();  // generic-proxy writes -> visible to the bulk (async) proxy
           __syncwarp();
           if (atomic) {
-            if (lane < 16 && !(p.probe & 16)) {
+            if (lane < 16 && !(probe & 16)) {
               // lane r ships row r: elements j0 .. j0+cnt-1 of input i = i0_w + r
               const int i = i0_w + lane;
               const int cnt = (i < p.n_inputs) ? min(32, min(i, p.n_inputs - 1) - j0 + 1) : 0;
@@ -119,7 +119,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
               bulk_commit();
             }
 
-          } else if (!(p.probe & 16)) {
+          } else if (!(probe & 16)) {
             // one packed-triangle row per instruction: 32 lanes x 8 B = 256 contiguous bytes
             const int j = j0 + lane;
             int i = i0_w;

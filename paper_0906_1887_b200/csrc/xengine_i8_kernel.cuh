@@ -28,7 +28,7 @@ __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_
   }
 }
 
-template <bool kPair>
+template <bool kPair, bool kProbe>
 __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, const CUtensorMap &tmap128,
                                                 const CUtensorMap &tmap64, const I8Params &p) {
   // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
@@ -41,6 +41,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
   uint64_t *acc_empty = acc_full + 2;
   uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(acc_empty + 2);
 
+  const int probe = kProbe ? p.probe : 0;  // diagnostics compile away in the production instantiation
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const int n_rounds = (p.n_items + p.units - 1) / p.units;
@@ -68,7 +69,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
 
   if (warp == 0) {
     // ===================================================================== TMA producer
-    if (lane == 0 && !(p.probe & 8)) {
+    if (lane == 0 && !(probe & 8)) {
       const uint64_t pol = policy_evict_normal();
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
@@ -81,7 +82,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
         for (int t = it.t0; t < it.t1; t += it.bk) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
-          if (p.probe & 2) {
+          if (probe & 2) {
             if (rank == 0) mbar_arrive(&full_bar[stage]);
           } else {
             // pair mode: both CTAs' boxes complete on the LEADER's barrier, which expects the bytes of both
@@ -134,19 +135,19 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         const uint32_t a_off = static_cast<uint32_t>(it.a_slot) * panel16;
         const uint32_t lbo_field = (panel16 & 0x3FFFu) << 16;
         const int n_chunks = (u_nblk + 1) >> 1;
-        if (!(p.probe & 4))
+        if (!(probe & 4))
           for (int q = 0; q < n_chunks; ++q) mbar_wait(&acc_empty[(ring + q) & 1], (((ring + q) >> 1) & 1) ^ 1);
         tc_fence_after();
         const uint32_t d0 = tmem_u + (ring & 1) * kAccCols;        // chunk 0
         const uint32_t d1 = tmem_u + ((ring + 1) & 1) * kAccCols;  // chunk 1
         const uint32_t idesc0 = u_nblk >= 2 ? kIdesc256 : kIdesc128;
         for (int t = u_t0; t < u_t1; t += u_bk) {
-          if (!(p.probe & 8)) mbar_wait(&full_bar[stage], phase);
+          if (!(probe & 8)) mbar_wait(&full_bar[stage], phase);
           tc_fence_after();
           const uint32_t lo_stage = (smem_lo + static_cast<uint32_t>(stage) * (p.stage_bytes >> 4)) | lbo_field;
           const int nk = (min(u_bk, u_t1 - t) + 31) >> 5;  // K = 32 samples per MMA; TMA zero-fills past T
           const uint32_t acc0 = (t != u_t0) ? 1u : 0u;  // the first MMA of the slice overwrites the accumulator
-          if (!(p.probe & 1)) {
+          if (!(probe & 1)) {
             if (p.diag) {
               for (int b = 0; b < u_nblk; ++b) {
                 const uint32_t dcol = ((b & 2) ? d1 : d0) + (b & 1) * 128;
@@ -162,7 +163,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
               else              issue_kn<kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0, nk);
             }
           }
-          if (leader && !(p.probe & 8)) {  // frees the stage (in both CTAs of a pair) when these MMAs retire
+          if (leader && !(probe & 8)) {  // frees the stage (in both CTAs of a pair) when these MMAs retire
             if (kPair) mma_commit_2sm(&empty_bar[stage], 3); else mma_commit(&empty_bar[stage]);
           }
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
@@ -174,12 +175,12 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         ring += n_chunks;
       }
     }
-  } else if (warp >= 4 && !(p.probe & 4)) {
+  } else if (warp >= 4 && !(probe & 4)) {
     // ===================================================================== epilogue
     const int ew = (warp - 4) & 3;   // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = (warp - 4) >> 2;  // which half (64 TMEM columns) of every block this warp folds
     i8_epilogue(p, tmem_base, smem + static_cast<size_t>(p.stages) * p.stage_bytes + (warp - 4) * kEpiWarpBytes,
-                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair);
+                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 
   tc_fence_before();
@@ -193,14 +194,16 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
 __global__ void __launch_bounds__(kI8Threads, 1)
 xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
                   const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  xengine_i8_body<false>(tmap256, tmap128, tmap64, p);
+  if (p.probe) xengine_i8_body<false, true>(tmap256, tmap128, tmap64, p);
+  else         xengine_i8_body<false, false>(tmap256, tmap128, tmap64, p);
 }
 
 // CTA pairs: tcgen05.mma.cta_group::2, M = 256 (one 128-row panel per CTA), each CTA stages half of B.
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kI8Threads, 1)
 xengine_i8_pair_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
                        const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  xengine_i8_body<true>(tmap256, tmap128, tmap64, p);
+  if (p.probe) xengine_i8_body<true, true>(tmap256, tmap128, tmap64, p);
+  else         xengine_i8_body<true, false>(tmap256, tmap128, tmap64, p);
 }
 
 }  // namespace corr
