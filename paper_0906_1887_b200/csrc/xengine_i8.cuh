@@ -15,13 +15,14 @@
 // kernel-parameter constant bank and is decoded with uniform arithmetic: everything the MMA issuer
 // touches stays in uniform registers, which is what lets one thread issue at the tensor-pipe rate.
 //
-// Warp roles (256 threads, 1 CTA/SM, persistent):
-//   warp 0   TMA producer: box {128 B along the chan*input axis, bk time rows}, SWIZZLE_128B.
+// Warp roles (384 threads, 1 CTA/SM, persistent):
+//   warp 8   TMA producer: box {128 B along the chan*input axis, bk time rows}, SWIZZLE_128B.
 //            This strided box load IS the corner turn: it lands as the
 //            canonical MN-major operand tile, so the input is read from HBM exactly once.
-//   warp 1   MMA issuer (one thread): tcgen05.mma.kind::i8, M=128, N=128|256, K=32.
-//   warp 2   TMEM allocator.
-//   warps 4-11 epilogue (two per TMEM lane quadrant, one per half block): tcgen05.ld, 2x2 fold via shfl.xor 1, packed-triangle stores (or integer
+//   warp 9   MMA issuer (one thread): tcgen05.mma.kind::i8, M=128, N=128|256, K=32.
+//   warp 10  TMEM allocator.
+//   warps 0-7 epilogue (two per TMEM lane quadrant, one per half block): tcgen05.ld, 2x2 fold via
+//            shfl.xor 1, packed-triangle stores (or integer
 //            red.add when an integration is split into time slices; integer sums are exact and
 //            order-independent, so the result stays bit-exact).
 #pragma once
@@ -31,6 +32,7 @@ namespace corr {
 
 constexpr int kI8Threads = 384;    // 4 control warps + 8 epilogue warps
 constexpr int kEpiWarps = 8;
+constexpr int kProducerWarp = 8, kMmaWarp = 9, kAllocWarp = 10;
 constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64 complex int8 samples
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
 constexpr int kMaxStages = 8;
