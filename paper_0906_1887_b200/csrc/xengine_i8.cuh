@@ -32,7 +32,7 @@ namespace corr {
 
 constexpr int kI8Threads = 384;    // 4 control warps + 8 epilogue warps
 constexpr int kEpiWarps = 8;
-constexpr int kProducerWarp = 8, kMmaWarp = 9, kAllocWarp = 10;
+constexpr int kProducerWarp = 8, kMmaWarp = 9, kAllocWarp = 10, kProducerWarp2 = 11;
 constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64 complex int8 samples
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
 constexpr int kMaxStages = 8;

@@ -70,8 +70,12 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
-  if (warp == kProducerWarp) {
-    // ===================================================================== TMA producer
+  if (warp == kProducerWarp || warp == kProducerWarp2) {
+    // ===================================================================== TMA producers
+    // two warps walk the same schedule and take alternate stages: one thread cannot issue the boxes of a
+    // stage (wait, expect_tx, up to 4 TMA instructions) as fast as the tensor pipe drains it
+    const int pw = (warp == kProducerWarp) ? 0 : 1;
+    int iter = 0;
     if (lane == 0 && !(probe & 8)) {
       const uint64_t pol = policy_evict_normal();
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
@@ -83,7 +87,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         const I8Item it = decode_item(p, cur, rank);
         const CUtensorMap *map = it.map == 0 ? &tmap256 : (it.map == 1 ? &tmap128 : &tmap64);
         const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
-        for (int t = it.t0; t < it.t1; t += it.bk) {
+        for (int t = it.t0; t < it.t1; t += it.bk, ++iter) {
+          if ((iter & 1) != pw) {
+            if (++stage == p.stages) { stage = 0; phase ^= 1; }
+            continue;
+          }
           mbar_wait(&empty_bar[stage], phase ^ 1);
           if (probe & 2) {
             if (rank == 0) mbar_arrive(&full_bar[stage]);

@@ -58,10 +58,12 @@ def run_cf32(pkg, x):
 
 # (N, C, T): several tiles + ragged tails; T in {1,31,32,33} pins K zero-padding (reading R11);
 # N=32 exercises the two-channels-per-panel mode incl. odd C; N=96/320/640 multi-panel, separate-A
-# and multi-segment items; N=1024 the c4 tile schedule.
+# and multi-segment items; N=1024 the c4 tile schedule (CTA pairs, cta_group::2).
 CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (64, 1, 257), (64, 200, 40),
               (32, 4, 100), (32, 3, 70), (32, 1, 64), (32, 301, 33), (96, 2, 64), (128, 2, 300),
-              (256, 2, 130), (320, 1, 64), (640, 1, 40), (1024, 1, 96)]
+              (256, 2, 130), (320, 1, 64), (640, 1, 40), (1024, 1, 96),
+              # CTA-pair kernel (N_I >= 512): even / odd panel counts, several stages, ragged T, many channels
+              (512, 3, 200), (576, 2, 70), (512, 40, 33), (2048, 1, 64)]
 
 
 @pytest.mark.parametrize("N,C,T", CI8_SHAPES)
