@@ -124,13 +124,22 @@ void plan_i8(corr_handle *h) {
     ip.n_panels = panels_per_chan;
     ip.n_groups = C;
     int k = 0;
-    if (h->use_pairs && panels_per_chan >= 8) {  // measured: pairs win from N_I = 512 up (c3, P = 4, loses 25 %)
-      // CTA pairs: 256 x 256 tiles (row-panel pair Ip, column-panel pair Jp <= Ip)
+    // CTA pairs (cta_group::2) from N_I = 512 up; already from N_I = 256 when the integration is long
+    // enough (T >= 2048) for 512-wide tiles, whose epilogue cannot overlap the next tile's MMAs
+    const bool wide_ok = T >= 2048 && panels_per_chan >= 4;
+    if (h->use_pairs && (panels_per_chan >= 8 || wide_ok)) {
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;
-      for (int Ip = pp - 1; Ip >= 0; --Ip)
-        for (int Jp = 0; Jp <= Ip; ++Jp) ip.kinds[k++] = static_cast<unsigned short>(Ip | (Jp << 6));
       max_load = 2;
+      for (int Ip = pp - 1; Ip >= 0; --Ip) {
+        const int ncols = 2 * Ip + 2;  // column panels 0 .. 2*Ip+1 are needed by row pair Ip
+        for (int J0 = 0; J0 < ncols;) {
+          const int wide = (wide_ok && ncols - J0 >= 4) ? 1 : 0;
+          ip.kinds[k++] = static_cast<unsigned short>(Ip | ((J0 >> 1) << 6) | (wide << 11));
+          if (wide) max_load = 3;
+          J0 += wide ? 4 : 2;
+        }
+      }
     } else {
       for (int I = panels_per_chan - 1; I >= 0; --I)
         for (int J0 = 0; J0 <= I; J0 += 2) {

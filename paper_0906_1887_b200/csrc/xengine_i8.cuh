@@ -59,13 +59,14 @@ struct I8Params {
   int probe;         // diagnostics only (corr_set_probe)
   long long n_baselines;
   int2 *vis;
-  unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11
+  unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11; pair: Ip | (J0 / 2) << 6 | wide << 11
 };
 
 struct I8Item {
   int t0, t1;        // time slice
   int nblk;          // 128-column blocks (1..4)
-  int nblk_load;     // B panels this CTA fetches (= nblk, except 1 in pair mode)
+  int nblk_load;     // B panels this CTA fetches (= nblk, except in pair mode)
+  int jperm;         // 1: TMEM column block b holds column panel J0 + {0, 2, 1, 3}[b] (512-wide pair tiles)
   int n_load;        // panels fetched per k-step (nblk, +1 when A is not one of the B panels)
   int a_slot;        // slab: smem slot of the A panel; diag: unused (A = B = slot b)
   int x0, z0;        // TMA coordinates of block 0 (block b at x0 + b*dx, z0 + b*dz)
@@ -121,18 +122,28 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
     else          { it.x0 = panel0 * kPanelBytes; it.z0 = 0; it.dx = kPanelBytes; it.dz = 0; }
     it.xa = 0; it.za = 0;
   } else if (p.pair2) {
-    // CTA `rank` of the pair owns row panel 2*Ip + rank and fetches column panel 2*Jp + rank (its half of B)
+    // CTA `rank` of the pair owns row panel 2*Ip + rank.  A 256-wide tile (wide = 0) puts column panel
+    // J0 + rank in this CTA (its half of B).  A 512-wide tile (wide = 1: two M=256,N=256 MMAs per k-step,
+    // all 512 TMEM columns) puts panels J0 + 2*rank, J0 + 2*rank + 1 here -- ADJACENT panels, so each
+    // time row is one 256..384-byte run in HBM -- which makes the TMEM column blocks hold the panels
+    // J0 + {0, 2, 1, 3}.  The A panel always gets its own slot so that both CTAs use the same offsets.
     const unsigned kd = p.kinds[k];
-    const int Ip = kd & 63, Jp = (kd >> 6) & 31;
-    it.I = 2 * Ip + rank; it.J0 = 2 * Jp; it.nblk = 2;
+    const int Ip = kd & 63;
+    const int wide = (kd >> 11) & 1;
+    it.I = 2 * Ip + rank; it.J0 = ((kd >> 6) & 31) * 2; it.nblk = wide ? 4 : 2;
+    it.jperm = wide;
     it.chan = grp;
-    const bool same = (Ip == Jp);  // diagonal tile: the CTA's A panel is its B half
-    it.n_load = same ? 1 : 2;
-    it.a_slot = same ? 0 : 1;
     const int xc = p.turned ? 0 : grp * row;
-    it.x0 = xc + (it.J0 + rank) * kPanelBytes; it.z0 = p.turned ? grp : 0; it.dx = 0; it.dz = 0;
+    it.z0 = p.turned ? grp : 0; it.dx = kPanelBytes; it.dz = 0;
     it.xa = xc + it.I * kPanelBytes; it.za = it.z0;
-    it.nblk_load = 1;
+    if (wide) {
+      it.nblk_load = 2; it.n_load = 3; it.a_slot = 2;
+      it.x0 = xc + (it.J0 + 2 * rank) * kPanelBytes;
+    } else {
+      const bool same = (2 * Ip == it.J0);  // diagonal tile: the CTA's A panel is its B half
+      it.nblk_load = 1; it.n_load = same ? 1 : 2; it.a_slot = same ? 0 : 1;
+      it.x0 = xc + (it.J0 + rank) * kPanelBytes;
+    }
   } else {
     const unsigned kd = p.kinds[k];
     it.I = kd & 63; it.J0 = ((kd >> 6) & 31) * 2; it.nblk = ((kd >> 11) & 1) + 1;
@@ -144,7 +155,7 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
     it.x0 = xc + it.J0 * kPanelBytes; it.z0 = p.turned ? grp : 0; it.dx = kPanelBytes; it.dz = 0;
     it.xa = xc + it.I * kPanelBytes; it.za = it.z0;
   }
-  if (!p.pair2) it.nblk_load = it.nblk;
+  if (!p.pair2) { it.nblk_load = it.nblk; it.jperm = 0; }
   if (it.n_load == 1)      { it.bk = 256; it.map = 0; }
   else if (it.n_load == 2) { it.bk = 128; it.map = 1; }
   else if (it.n_load == 3 && p.stage_bytes >= 3 * 128 * kPanelBytes) { it.bk = 128; it.map = 1; }

@@ -39,7 +39,8 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
       const int nb_here = min(2, it.nblk - 2 * q);
       for (int bb = 0; bb < nb_here; ++bb) {
         const int b = 2 * q + bb;
-        if (!p.diag && it.J0 + b > it.I) continue;  // block above the diagonal (pair tiles on the diagonal)
+        const int Jb = it.J0 + (it.jperm ? (((b & 1) << 1) | (b >> 1)) : b);  // column panel held by block b
+        if (!p.diag && Jb > it.I) continue;  // block above the diagonal (pair tiles on the diagonal)
         // what this warp's 16 rows and the block's 64 column-inputs are (all warp-uniform)
         int chan_w, i0_w, j_blk0;
         bool diag_blk;
@@ -52,8 +53,8 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
         } else {
           chan_w = it.chan;
           i0_w = it.I * 64 + ew * 16;
-          j_blk0 = (it.J0 + b) * 64;
-          diag_blk = (it.J0 + b) == it.I;
+          j_blk0 = Jb * 64;
+          diag_blk = Jb == it.I;
         }
         const bool warp_ok = (chan_w < p.n_chan) && (i0_w < p.n_inputs);
         // this lane pair's row: input i_row, its first packed element and how many columns it keeps

@@ -172,6 +172,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
               else if (nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else if (nk == 8) issue_k<8, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else              issue_kn<kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0, nk);
+              if (kPair && u_nblk > 2) {  // 512-wide pair tile: second column half from smem slot 1 into chunk 1
+                const uint32_t lo_b1 = lo_stage + panel16;
+                if (nk == 4) issue_k<4, kPair>(d1, lo_a, lo_b1, kDescHi, idesc0, acc0);
+                else         issue_kn<kPair>(d1, lo_a, lo_b1, kDescHi, idesc0, acc0, nk);
+              }
             }
           }
           if (leader && !(probe & 8)) {  // frees the stage (in both CTAs of a pair) when these MMAs retire

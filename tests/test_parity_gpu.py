@@ -63,7 +63,9 @@ CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (
               (32, 4, 100), (32, 3, 70), (32, 1, 64), (32, 301, 33), (96, 2, 64), (128, 2, 300),
               (256, 2, 130), (320, 1, 64), (640, 1, 40), (1024, 1, 96),
               # CTA-pair kernel (N_I >= 512): even / odd panel counts, several stages, ragged T, many channels
-              (512, 3, 200), (576, 2, 70), (512, 40, 33), (2048, 1, 64)]
+              (512, 3, 200), (576, 2, 70), (512, 40, 33), (2048, 1, 64),
+              # long integrations (T >= 2048): 512-wide pair tiles from N_I = 256 up, mixed with 256-wide ones
+              (256, 3, 2100), (320, 1, 2050), (512, 1, 2081)]
 
 
 @pytest.mark.parametrize("N,C,T", CI8_SHAPES)
