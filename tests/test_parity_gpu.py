@@ -82,6 +82,15 @@ def test_ci8_uniform_full_range_bit_exact(pkg, N, C, T):
     assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
 
 
+@pytest.mark.parametrize("N,C,T", [(512, 2, 100), (256, 2, 2100), (1024, 1, 64)])
+def test_ci8_single_cta_slabs_when_pairs_are_disabled(pkg, N, C, T, monkeypatch):
+    """CORR_NO_PAIRS=1 (the A/B knob of DESIGN.md section 11) selects the single-CTA slab schedule."""
+    monkeypatch.setenv("CORR_NO_PAIRS", "1")
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+
+
 def test_ci8_zero_input(pkg):
     x = np.zeros((40, 3, 64, 2), np.int8)
     assert not run_ci8(pkg, x).any()
@@ -96,7 +105,7 @@ def test_ci8_extreme_constant_longest_integration(pkg, val):
     assert out[..., 0].max() == 65535 * 2 * val * val
 
 
-@pytest.mark.parametrize("N,C,T", [(64, 6, 100), (32, 4, 70), (256, 2, 64), (96, 2, 40)])
+@pytest.mark.parametrize("N,C,T", [(64, 6, 100), (32, 4, 70), (256, 2, 64), (96, 2, 40), (512, 2, 70), (256, 1, 2100)])
 def test_ci8_standalone_corner_turn_path(pkg, N, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
