@@ -71,22 +71,23 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
           const int par = atomic ? static_cast<int>((static_cast<long long>(chan_w) * p.n_baselines +
                                                       i_row * (i_row + 1) / 2 + j0) & 1) : 0;
           int *st_row = st_w + par * 2;
-          uint32_t v[32];
-          tmem_ld_32x32(tchunk + bb * 128 + h * 64, v);
-          // the previous half block's bulk stores must have read the staging buffer before it is reused
+          // both 32-column loads of the half block are in flight before the single wait
+          uint32_t v0[32], v1[32];
+          tmem_ld_32x32(tchunk + bb * 128 + h * 64, v0);
+          tmem_ld_32x32(tchunk + bb * 128 + h * 64 + 32, v1);
           if (atomic && lane < 16) bulk_wait_read_all();  // earlier bulk reduces have read the staging buffer
-          __syncwarp();
+          __syncwarp();  // the previous half block has been read out of the staging buffer
+          tmem_ld_wait();
 #pragma unroll
-          for (int cb = 0; cb < 2; ++cb) {
-            if (cb == 1) tmem_ld_32x32(tchunk + bb * 128 + h * 64 + 32, v);
-            tmem_ld_wait();
-#pragma unroll
-            for (int jj = 0; jj < 16; ++jj) {
-              const int other = __shfl_xor_sync(0xffffffffu, static_cast<int>(v[2 * jj + 1]), 1);
-              int val = part ? (static_cast<int>(v[2 * jj]) - other) : (static_cast<int>(v[2 * jj]) + other);
-              if (part && (j0 + cb * 16 + jj) == i_row) val = 0;  // Im of an autocorrelation is exactly 0
-              st_row[(cb * 16 + jj) * 2] = val;                   // even lane: Re -> .x, odd lane: Im -> .y
-            }
+          for (int jj = 0; jj < 16; ++jj) {
+            const int o0 = __shfl_xor_sync(0xffffffffu, static_cast<int>(v0[2 * jj + 1]), 1);
+            const int o1 = __shfl_xor_sync(0xffffffffu, static_cast<int>(v1[2 * jj + 1]), 1);
+            int a0 = part ? (static_cast<int>(v0[2 * jj]) - o0) : (static_cast<int>(v0[2 * jj]) + o0);
+            int a1 = part ? (static_cast<int>(v1[2 * jj]) - o1) : (static_cast<int>(v1[2 * jj]) + o1);
+            if (part && (j0 + jj) == i_row) a0 = 0;       // Im of an autocorrelation is exactly 0
+            if (part && (j0 + 16 + jj) == i_row) a1 = 0;
+            st_row[jj * 2] = a0;                          // even lane: Re -> .x, odd lane: Im -> .y
+            st_row[(16 + jj) * 2] = a1;
           }
           if (atomic) fence_proxy_async();  // generic-proxy writes -> visible to the bulk (async) proxy
           __syncwarp();
@@ -126,13 +127,14 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
             int i = i0_w;
             int2 *row = p.vis + (static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j);
             const int2 *src = reinterpret_cast<const int2 *>(stage_buf) + lane;
-#pragma unroll 4
+            int2 val[16];
+#pragma unroll
+            for (int rr = 0; rr < 16; ++rr) val[rr] = src[rr * (kEpiRowBytes / 8)];  // 16 independent loads
+#pragma unroll
             for (int rr = 0; rr < 16; ++rr) {
-              if (i >= p.n_inputs) break;
-              const int2 val = src[rr * (kEpiRowBytes / 8)];
-              if (j <= i && j < p.n_inputs) {
-                if (atomic) put_vis<true>(row, val.x, val.y);
-                else        put_vis<false>(row, val.x, val.y);
+              if (i < p.n_inputs && j <= i && j < p.n_inputs) {
+                if (atomic) put_vis<true>(row, val[rr].x, val[rr].y);
+                else        put_vis<false>(row, val[rr].x, val[rr].y);
               }
               ++i;
               row += i;  // next row of the triangle starts i+1 elements further on
