@@ -76,7 +76,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     // stage (wait, expect_tx, up to 4 TMA instructions) as fast as the tensor pipe drains it
     const int pw = (warp == kProducerWarp) ? 0 : 1;
     int iter = 0;
-    if (lane == 0 && !(probe & 8)) {
+    if (elect_one() && !(probe & 8)) {
       const uint64_t pol = policy_evict_normal();
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
@@ -122,7 +122,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     // The whole warp walks the (uniform) schedule so that loop state lives in uniform registers;
     // one lane issues.  Descriptor low words are advanced by plain adds (all offsets are multiples
     // of 16 B and the address field cannot carry into the LBO field below 256 KB).
-    if (lane == 0 && rank == 0) {
+    if (rank == 0 && elect_one()) {
       constexpr bool leader = true;
       int stage = 0;
       uint32_t phase = 0;
@@ -154,7 +154,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         const uint32_t idesc0 = u_nblk >= 2 ? kIdesc256 : kIdesc128;
         for (int t = u_t0; t < u_t1; t += u_bk) {
           if (!(probe & 8)) mbar_wait(&full_bar[stage], phase);
-          tc_fence_after();
+          if (!(kProbe && (probe & 64))) tc_fence_after();
           const uint32_t lo_stage = (smem_lo + static_cast<uint32_t>(stage) * (p.stage_bytes >> 4)) | lbo_field;
           const int nk = (min(u_bk, u_t1 - t) + 31) >> 5;  // K = 32 samples per MMA; TMA zero-fills past T
           const uint32_t acc0 = (t != u_t0) ? 1u : 0u;  // the first MMA of the slice overwrites the accumulator
@@ -168,6 +168,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
               }
             } else {
               const uint32_t lo_a = lo_stage + a_off;
+              if (kProbe && (probe & 32) && nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);  // diagnostics: issue twice
               if (nk == 2)      issue_k<2, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else if (nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else if (nk == 8) issue_k<8, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
