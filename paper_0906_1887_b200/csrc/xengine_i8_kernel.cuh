@@ -119,9 +119,9 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     }
   } else if (warp == kMmaWarp) {
     // ===================================================================== MMA issuer
-    // The whole warp walks the (uniform) schedule so that loop state lives in uniform registers;
-    // one lane issues.  Descriptor low words are advanced by plain adds (all offsets are multiples
-    // of 16 B and the address field cannot carry into the LBO field below 256 KB).
+    // One elected thread (elect.sync, so that ptxas emits plain uniform-datapath code without a waterfall
+    // loop around every UTCIMMA) walks the schedule.  Descriptor low words are advanced by plain adds
+    // (all offsets are multiples of 16 B and the address field cannot carry into the LBO field below 256 KB).
     if (rank == 0 && elect_one()) {
       constexpr bool leader = true;
       int stage = 0;
@@ -136,8 +136,6 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
         const I8Item it = decode_item(p, cur, 0);
-        // decode_item divides, so its results sit in vector registers; one REDUX each brings what the
-        // issue loop needs into uniform registers (an R2UR in front of every MMA costs ~60 cycles).
         const int u_bk = it.bk;
         const int u_t0 = it.t0;
         const int u_t1 = it.t1;
