@@ -65,7 +65,9 @@ CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (
               # CTA-pair kernel (N_I >= 512): even / odd panel counts, several stages, ragged T, many channels
               (512, 3, 200), (576, 2, 70), (512, 40, 33), (2048, 1, 64),
               # long integrations (T >= 2048): 512-wide pair tiles from N_I = 256 up, mixed with 256-wide ones
-              (256, 3, 2100), (320, 1, 2050), (512, 1, 2081)]
+              (256, 3, 2100), (320, 1, 2050), (512, 1, 2081),
+              # the largest N_I the ABI admits (528 schedule kinds per channel)
+              (4096, 1, 40)]
 
 
 @pytest.mark.parametrize("N,C,T", CI8_SHAPES)
