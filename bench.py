@@ -202,7 +202,10 @@ def run_reference(args, w):
     t0 = time.perf_counter()
     fn(x, 0, 1, threads=1)
     one = max(time.perf_counter() - t0, 1e-4)
-    k = int(min(w.n_chan, max(cores, 2.0 * cores / one)))   # about 2 s of work per step
+    # bounded sample: about 2 s of work per step, less when many steps are asked for, so that the whole
+    # --steps K --warmup W run stays within ~2 minutes
+    step_s = min(2.0, 120.0 / max(1, args.steps + args.warmup))
+    k = int(min(w.n_chan, max(1, step_s * cores / one)))
     for _ in range(args.warmup):
         fn(x, 0, k, threads=cores)
     t0 = time.perf_counter()
