@@ -95,9 +95,11 @@ int corr_launches_per_call(const corr_handle *h);
 int corr_set_turn(corr_handle *h, int mode);
 
 /*
- * corr_set_probe -- DIAGNOSTICS ONLY (results are garbage while a probe is on): CI8 kernel with
- * 1 = MMAs skipped (measures the TMA fill rate), 2 = TMA loads skipped (measures the MMA issue
- * rate), 0 = normal.  Used by the roofline study in DESIGN.md, never by tests of results.
+ * corr_set_probe -- DIAGNOSTICS ONLY (results are garbage while a probe is on): switches engines of the CI8
+ * kernel off so that the others can be timed alone.  Bit mask: 1 = skip the MMAs, 2 = skip the TMA loads
+ * (producer only hand-shakes), 4 = no epilogue, 8 = no producer and no stage hand-shake at all, 16 = epilogue
+ * without its global stores; 0 = normal (the production instantiation has none of this code).  Used by the
+ * roofline study in DESIGN.md section 7, never by tests of results.
  */
 int corr_set_probe(corr_handle *h, int mode);
 

@@ -90,3 +90,20 @@ def test_product_and_oracle_are_independent():
             pre = src[:m.start()]
             fn = re.findall(r"^def (\w+)", pre, flags=re.M)[-1]
             assert fn in ("cpu_baseline", "run_reference"), f"bench.py imports oracle inside {fn}()"
+
+
+@needs_nvcc
+def test_sass_is_blackwell_native():
+    """The built library carries tcgen05 MMAs (UTCIMMA, incl. the 2-CTA form), TMEM loads (LDTM) and TMA
+    (UTMALDG) in its SASS, and no legacy tensor path (HMMA/IMMA warp-level MMAs)."""
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump not available")
+    import subprocess
+    import paper_0906_1887_b200 as pkg
+    pkg.lib()
+    lib = os.path.join(ROOT, "paper_0906_1887_b200", "libcorr.so")
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, timeout=300).stdout
+    assert "sm_100a" in sass
+    for mnemonic in ("UTCIMMA", "UTCIMMA.2CTA", "LDTM", "UTMALDG", "UTCBAR"):
+        assert mnemonic in sass, f"{mnemonic} missing from the SASS"
+    assert " HMMA" not in sass and " IMMA" not in sass

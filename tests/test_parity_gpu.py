@@ -205,3 +205,11 @@ def test_abi_errors_on_device(pkg):
         with pytest.raises(pkg.CorrError):
             pkg.corr_create(*bad)
     assert L.corr_destroy(None) == pkg.CORR_OK
+
+
+def test_mma_probe_runs_at_the_tensor_rate(pkg):
+    """corr_probe_mma: one thread per SM issues M=128,N=256,K=32 int8 MMAs back to back; the tensor pipe needs
+    128 cycles for each (8192 MACs per cycle per SM), MN-major operands included."""
+    r = pkg.probe_mma(128, 256, True, 8192, random_fill=True)
+    assert 120.0 <= r["cycles_per_mma"] <= 150.0, r
+    assert r["tops"] > 3000.0, r
