@@ -173,6 +173,17 @@ def gauss_f32_numpy(T, C, N, seed, sigma, tone_amp=0.0, t_begin=0, t_end=None):
     return out
 
 
+def pack_ci4(x):
+    """int8 cube [T][C][N][2] with values in [-8, 7] -> uint8 [T][C][N], one byte per complex sample:
+    low nibble = Re, high nibble = Im, two's complement (the paper's "1-byte mode").
+    Input generation only: no method arithmetic."""
+    x = np.asarray(x)
+    if x.dtype != np.int8 or x.shape[-1] != 2 or x.min() < -8 or x.max() > 7:
+        raise ValueError("pack_ci4 needs int8 [...][2] with values in [-8, 7]")
+    u = x.view(np.uint8)
+    return ((u[..., 0] & 15) | ((u[..., 1] & 15) << 4)).astype(np.uint8)
+
+
 # --------------------------------------------------------------------------- workloads
 
 @dataclass(frozen=True)

@@ -7,7 +7,7 @@ package.  The product package never does (tests/test_independence.py checks).
 All arithmetic is in ``xcorr_oracle.c`` (read its header for the passages it
 follows: PAPER.md:47, :53, :84, :107, :115).  This file only marshals numpy
 arrays.  Parity status: every function below is pinned by
-``tests/test_oracle_pins.py`` (P1-P9, tests/golden/); none is "parity unpinned".
+``tests/test_oracle_pins.py`` (P1-P9, P11-P12 for the 4-bit mode, tests/golden/); none is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -45,6 +45,9 @@ def _load():
         L, I, P = ctypes.c_long, ctypes.c_int, ctypes.c_void_p
         _lib.oracle_xengine_ci8.argtypes = [P, L, L, L, L, L, P, I]
         _lib.oracle_xengine_cf32.argtypes = [P, L, L, L, L, L, P, I]
+        _lib.oracle_xengine_ci4.argtypes = [P, L, L, L, L, L, P, I]
+        _lib.oracle_unpack_ci4.argtypes = [ctypes.c_ubyte, ctypes.POINTER(I), ctypes.POINTER(I)]
+        _lib.oracle_unpack_ci4.restype = None
         _lib.oracle_full_matrix_ci8.argtypes = [P, L, L, L, L, P]
         _lib.oracle_full_matrix_cf32.argtypes = [P, L, L, L, L, P]
         _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
@@ -71,6 +74,27 @@ def xengine_ci8(x, c_begin=0, c_end=None, threads=1):
     rc = _load().oracle_xengine_ci8(x.ctypes.data, T, C, N, c_begin, c_end, vis.ctypes.data, threads)
     if rc == -2:
         raise OracleOverflow("visibility does not fit int32")
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return vis
+
+
+def unpack_ci4(byte):
+    """(re, im) of one packed 4+4-bit sample (reading R18: low nibble Re, high nibble Im, two's complement)."""
+    re, im = ctypes.c_int(), ctypes.c_int()
+    _load().oracle_unpack_ci4(int(byte) & 255, ctypes.byref(re), ctypes.byref(im))
+    return re.value, im.value
+
+
+def xengine_ci4(x, c_begin=0, c_end=None, threads=1):
+    """x: uint8 [T][C][N] packed 4+4-bit samples -> int32 [c_end-c_begin][N(N+1)/2][2]."""
+    x = np.ascontiguousarray(x)
+    if x.dtype != np.uint8 or x.ndim != 3:
+        raise ValueError(f"expected [T][C][N] uint8, got {x.dtype} {x.shape}")
+    T, C, N = x.shape
+    c_end = C if c_end is None else c_end
+    vis = np.empty((c_end - c_begin, N * (N + 1) // 2, 2), dtype=np.int32)
+    rc = _load().oracle_xengine_ci4(x.ctypes.data, T, C, N, c_begin, c_end, vis.ctypes.data, threads)
     if rc != 0:
         raise MemoryError("oracle allocation failed")
     return vis

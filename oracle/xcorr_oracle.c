@@ -198,3 +198,52 @@ int oracle_one_visibility_cf32(const float *x, long n_time, long n_chan, long n_
     re_im[1] = im;
     return ORACLE_OK;
 }
+
+/*
+ * 4-bit packed input: the paper's "1-byte mode" ("4+4 bits ... halves the volume";
+ * samples are two's complement).  Reading R18: one byte per complex sample,
+ * LOW nibble = Re, HIGH nibble = Im, each a two's-complement 4-bit integer in [-8, 7].
+ * The visibilities are the same definition as above applied to the unpacked values.
+ */
+static int nibble_to_int(unsigned v /* 0..15 */) { return v >= 8 ? (int)v - 16 : (int)v; }
+
+void oracle_unpack_ci4(uint8_t byte, int *re, int *im)
+{
+    *re = nibble_to_int(byte & 15u);
+    *im = nibble_to_int((unsigned)byte >> 4);
+}
+
+int oracle_xengine_ci4(const uint8_t *x, long n_time, long n_chan, long n_inputs,
+                       long c_begin, long c_end, int32_t *vis, int threads)
+{
+    const long nb = n_inputs * (n_inputs + 1) / 2;
+    int status = ORACLE_OK;
+    (void)threads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads > 1 ? threads : 1)
+    for (long c = c_begin; c < c_end; ++c) {
+        int64_t *acc = (int64_t *)calloc((size_t)(2 * nb), sizeof(int64_t));
+        if (!acc) {
+#pragma omp critical
+            status = ORACLE_EALLOC;
+            continue;
+        }
+        for (long t = 0; t < n_time; ++t) {
+            const uint8_t *xt = x + (t * n_chan + c) * n_inputs;
+            long b = 0;
+            for (long i = 0; i < n_inputs; ++i) {
+                int ai, bi;
+                oracle_unpack_ci4(xt[i], &ai, &bi);
+                for (long j = 0; j <= i; ++j, ++b) {
+                    int aj, bj;
+                    oracle_unpack_ci4(xt[j], &aj, &bj);
+                    acc[2 * b] += (int64_t)ai * aj + (int64_t)bi * bj;     /* Re x_i conj(x_j) */
+                    acc[2 * b + 1] += (int64_t)bi * aj - (int64_t)ai * bj; /* Im x_i conj(x_j) */
+                }
+            }
+        }
+        int32_t *out = vis + 2 * nb * (c - c_begin);
+        for (long k = 0; k < 2 * nb; ++k) out[k] = (int32_t)acc[k]; /* |V| <= T*2*64 always fits */
+        free(acc);
+    }
+    return status;
+}
