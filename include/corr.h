@@ -36,7 +36,10 @@ typedef struct corr_handle corr_handle; /* opaque */
 
 /* dtype of the voltage samples */
 enum { CORR_CI8 = 0,   /* (int8 re, int8 im) -> (int32 re, int32 im), exact            */
-       CORR_CF32 = 1   /* (float re, float im) -> (float re, float im), FP32 FMA sums  */ };
+       CORR_CF32 = 1,  /* (float re, float im) -> (float re, float im), FP32 FMA sums  */
+       CORR_CI4 = 2    /* one byte per sample: low nibble Re, high nibble Im, 4-bit two's
+                          complement (the paper's "1-byte mode"; DESIGN R18)
+                          -> (int32 re, int32 im), exact; d_in is [n_time][n_chan][n_inputs] bytes */ };
 
 /* status codes */
 enum { CORR_OK = 0, CORR_EINVAL = 1, CORR_EUNSUPPORTED = 2, CORR_EALLOC = 3,
@@ -82,7 +85,7 @@ const char *corr_last_error(void);
 int corr_last_status(void);
 
 /* Sizes in bytes of one integration's input and output for this handle. */
-size_t corr_in_bytes(const corr_handle *h);  /* T*C*N*2 (CI8) or T*C*N*8 (CF32) */
+size_t corr_in_bytes(const corr_handle *h);  /* T*C*N*2 (CI8), T*C*N (CI4) or T*C*N*8 (CF32) */
 size_t corr_vis_bytes(const corr_handle *h); /* C*N(N+1)/2*8                    */
 
 /* Number of kernel launches one corr_xengine call enqueues (for bench accounting). */

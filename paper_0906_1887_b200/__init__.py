@@ -12,7 +12,7 @@ import os
 
 from . import build as _build
 
-CORR_CI8, CORR_CF32 = 0, 1
+CORR_CI8, CORR_CF32, CORR_CI4 = 0, 1, 2
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
 CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 
@@ -74,7 +74,7 @@ class Correlator:
 
     def __init__(self, n_inputs, n_chan, n_time, dtype):
         self.n_inputs, self.n_chan, self.n_time = n_inputs, n_chan, n_time
-        self.dtype = {"ci8": CORR_CI8, "cf32": CORR_CF32}.get(dtype, dtype)
+        self.dtype = {"ci8": CORR_CI8, "cf32": CORR_CF32, "ci4": CORR_CI4}.get(dtype, dtype)
         self._h = lib().corr_create(n_inputs, n_chan, n_time, self.dtype)
         if not self._h:
             _raise()
@@ -100,7 +100,7 @@ class Correlator:
 
     def empty_vis(self, n=1):
         import torch
-        dt = torch.int32 if self.dtype == CORR_CI8 else torch.float32
+        dt = torch.float32 if self.dtype == CORR_CF32 else torch.int32
         shape = (self.n_chan, self.n_baselines, 2) if n == 1 else (n, self.n_chan, self.n_baselines, 2)
         return torch.empty(shape, dtype=dt, device="cuda")
 

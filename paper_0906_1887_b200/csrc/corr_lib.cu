@@ -157,9 +157,10 @@ void plan_i8(corr_handle *h) {
   // 32 KB stages: 1 x 256, 2 x 128 or 4 x 64 time rows of 128 B; 48 KB when items fetch 3 panels (3 x 128)
   ip.stage_bytes = (!ip.diag && max_load == 3) ? 3 * 128 * 128 : 4 * 64 * 128;
   const int epi_bytes = corr::kEpiWarps * corr::kEpiWarpBytes;  // epilogue staging behind the stage ring
-  const int bar_bytes = 256;  // 2 * kMaxStages + 4 mbarriers and the TMEM base address
-  ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ip.stage_bytes);
-  h->smem_i8 = static_cast<size_t>(ip.stage_bytes) * ip.stages + epi_bytes + bar_bytes;
+  const int bar_bytes = 512;  // 4 * kMaxStages + 4 mbarriers and the TMEM base address
+  const int ring_bytes = h->dtype == CORR_CI4 ? ip.stage_bytes * 3 / 2 : ip.stage_bytes;  // + packed (raw) ring
+  ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ring_bytes);
+  h->smem_i8 = static_cast<size_t>(ring_bytes) * ip.stages + epi_bytes + bar_bytes;
   ip.units = std::min(ip.n_items, ip.pair2 ? h->n_sms / 2 : h->n_sms);
   h->grid_i8 = ip.pair2 ? 2 * ip.units : ip.units;
   const int deltas[2] = {ip.units + ip.rot, ip.rot};
@@ -178,15 +179,16 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
 int encode_map(corr_handle *h, const void *base, bool turned, int box_rows, CUtensorMap *out) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return fail(CORR_ECUDA, "cuTensorMapEncodeTiled entry point not available");
-  const cuuint64_t row = static_cast<cuuint64_t>(2) * h->n_inputs;  // bytes per (t, c)
+  const bool packed = h->dtype == CORR_CI4;  // one byte per sample, 64-byte boxes, no swizzle (expanded in smem)
+  const cuuint64_t row = static_cast<cuuint64_t>(packed ? 1 : 2) * h->n_inputs;  // bytes per (t, c)
   CUresult r;
   if (!turned) {
     cuuint64_t dims[2] = {row * h->n_chan, static_cast<cuuint64_t>(h->n_time)};
     cuuint64_t strides[1] = {row * h->n_chan};
-    cuuint32_t box[2] = {128, static_cast<cuuint32_t>(box_rows)};
+    cuuint32_t box[2] = {packed ? 64u : 128u, static_cast<cuuint32_t>(box_rows)};
     cuuint32_t es[2] = {1, 1};
     r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), dims, strides, box, es,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, packed ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   } else {
     const cuuint64_t grow = h->pair_mode ? 2 * row : row;
@@ -234,7 +236,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
     fail(CORR_EINVAL, "corr_create: n_inputs, n_chan, n_time must be positive (got %d, %d, %d)", n_inputs, n_chan, n_time);
     return nullptr;
   }
-  if (dtype != CORR_CI8 && dtype != CORR_CF32) {
+  if (dtype != CORR_CI8 && dtype != CORR_CF32 && dtype != CORR_CI4) {
     fail(CORR_EINVAL, "corr_create: unknown dtype %d", dtype);
     return nullptr;
   }
@@ -242,7 +244,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
     fail(CORR_EUNSUPPORTED, "corr_create: n_inputs must be a multiple of 32 and <= 4096 (got %d)", n_inputs);
     return nullptr;
   }
-  if (dtype == CORR_CI8 && n_time > 65535) {
+  if (dtype != CORR_CF32 && n_time > 65535) {
     fail(CORR_EUNSUPPORTED, "corr_create: CI8 needs n_time <= 65535 so that int32 cannot overflow (got %d)", n_time);
     return nullptr;
   }
@@ -270,7 +272,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->n_time = n_time;
   h->dtype = dtype;
   h->n_baselines = static_cast<long long>(n_inputs) * (n_inputs + 1) / 2;
-  h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * (dtype == CORR_CI8 ? 2 : 8);
+  h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * (dtype == CORR_CI8 ? 2 : dtype == CORR_CI4 ? 1 : 8);
   h->vis_bytes = static_cast<size_t>(n_chan) * h->n_baselines * 8;
   h->n_sms = prop.multiProcessorCount;
   h->turn_mode = CORR_TURN_FUSED;
@@ -281,10 +283,12 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->s_copy = h->s_compute = nullptr;
 
   cudaError_t e = cudaSuccess;
-  if (dtype == CORR_CI8) {
-    h->use_pairs = getenv("CORR_NO_PAIRS") ? 0 : 1;  // CTA pairs (cta_group::2) for N_I >= 128
+  if (dtype != CORR_CF32) {
+    h->use_pairs = (dtype == CORR_CI4 || getenv("CORR_NO_PAIRS")) ? 0 : 1;  // the 4-bit path is single-CTA only  // CTA pairs (cta_group::2) for N_I >= 128
     plan_i8(h);
     e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(corr::xengine_i4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(corr::xengine_i8_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
   } else {
@@ -407,6 +411,7 @@ int corr_corner_turn(corr_handle *h, const void *d_in, void *d_out, void *stream
   if ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_out)) & 15)
     return fail(CORR_EINVAL, "corr_corner_turn: pointers must be 16-byte aligned");
   if (d_in == d_out) return fail(CORR_EINVAL, "corr_corner_turn: d_in and d_out alias");
+  if (h->dtype == CORR_CI4) return fail(CORR_EUNSUPPORTED, "corr_corner_turn: not provided for the 4-bit packed input");
   if (h->dtype == CORR_CI8 && h->pair_mode && (h->n_chan & 1))
     return fail(CORR_EUNSUPPORTED, "corr_corner_turn: n_inputs == 32 needs an even n_chan");
   return launch_turn(h, d_in, d_out, static_cast<cudaStream_t>(stream));
@@ -447,8 +452,10 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.turned = turned ? 1 : 0;
   ip.vis = static_cast<int2 *>(d_vis);
   ip.probe = h->probe;
+  ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
   if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
-  if (ip.pair2) corr::xengine_i8_pair_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+  if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<h->grid_i8, corr::kI4Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+  else if (ip.pair2) corr::xengine_i8_pair_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   else          corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;

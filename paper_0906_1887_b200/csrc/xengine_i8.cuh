@@ -32,6 +32,8 @@ namespace corr {
 
 constexpr int kI8Threads = 384;    // 4 control warps + 8 epilogue warps
 constexpr int kEpiWarps = 8;
+constexpr int kExpandWarp0 = 12, kExpandWarps = 4;  // 4-bit input only (512-thread launch)
+constexpr int kI4Threads = 512;
 constexpr int kProducerWarp = 8, kMmaWarp = 9, kAllocWarp = 10, kProducerWarp2 = 11;
 constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64 complex int8 samples
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
@@ -57,6 +59,7 @@ struct I8Params {
   int stages, stage_bytes;
   int turned;        // 0: d_in is [T][C][2N] (2-D maps); 1: scratch is [G][T][W] (3-D maps)
   int probe;         // diagnostics only (corr_set_probe)
+  int out_shift;     // 8 for 4-bit input (operands are 16 x the samples), else 0
   long long n_baselines;
   int2 *vis;
   unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11; pair: Ip | (J0 / 2) << 6 | wide << 11

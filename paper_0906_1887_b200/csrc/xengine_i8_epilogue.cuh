@@ -24,6 +24,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
   const bool atomic = p.n_slices > 1;
+  const int out_shift = p.out_shift;
   int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kEpiRowBytes / 4) + part;
   uint32_t ring = 0;
   I8Iter cur = iter_init(p);
@@ -84,6 +85,8 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
             const int o1 = __shfl_xor_sync(0xffffffffu, static_cast<int>(v1[2 * jj + 1]), 1);
             int a0 = part ? (static_cast<int>(v0[2 * jj]) - o0) : (static_cast<int>(v0[2 * jj]) + o0);
             int a1 = part ? (static_cast<int>(v1[2 * jj]) - o1) : (static_cast<int>(v1[2 * jj]) + o1);
+            a0 >>= out_shift;  // 4-bit input: sums are exact multiples of 256
+            a1 >>= out_shift;
             if (part && (j0 + jj) == i_row) a0 = 0;       // Im of an autocorrelation is exactly 0
             if (part && (j0 + 16 + jj) == i_row) a1 = 0;
             st_row[jj * 2] = a0;                          // even lane: Re -> .x, odd lane: Im -> .y

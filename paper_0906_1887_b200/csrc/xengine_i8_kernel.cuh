@@ -28,18 +28,24 @@ __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_
   }
 }
 
-template <bool kPair, bool kProbe>
+template <bool kPair, bool kProbe, bool kPacked = false>
 __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, const CUtensorMap &tmap128,
                                                 const CUtensorMap &tmap64, const I8Params &p) {
   // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
   // 128-byte swizzle needs: [stage ring][epilogue staging][mbarriers + TMEM base].
   extern __shared__ __align__(1024) uint8_t smem[];
-  uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(p.stages) * p.stage_bytes +
-                                                    kEpiWarps * kEpiWarpBytes);
+  // 4-bit packed input (kPacked): TMA lands the packed boxes in a second ring (half the bytes) behind the
+  // int8 ring; four expand warps sign-extend the nibbles into the int8 ring in the MN-major SW128 layout.
+  const uint32_t raw_stage_bytes = kPacked ? static_cast<uint32_t>(p.stage_bytes) / 2 : 0;
+  uint8_t *raw = smem + static_cast<size_t>(p.stages) * p.stage_bytes;
+  uint8_t *epi_stage = raw + static_cast<size_t>(p.stages) * raw_stage_bytes;
+  uint64_t *full_bar = reinterpret_cast<uint64_t *>(epi_stage + kEpiWarps * kEpiWarpBytes);
   uint64_t *empty_bar = full_bar + kMaxStages;
   uint64_t *acc_full = empty_bar + kMaxStages;
   uint64_t *acc_empty = acc_full + 2;
-  uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(acc_empty + 2);
+  uint64_t *raw_full = acc_empty + 2;
+  uint64_t *raw_empty = raw_full + kMaxStages;
+  uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(raw_empty + kMaxStages);
 
   const int probe = kProbe ? p.probe : 0;  // diagnostics compile away in the production instantiation
   const int warp = threadIdx.x >> 5;
@@ -55,8 +61,12 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     tma_prefetch_desc(&tmap128);
     tma_prefetch_desc(&tmap64);
     for (int s = 0; s < p.stages; ++s) {
-      mbar_init(&full_bar[s], 1);
+      mbar_init(&full_bar[s], kPacked ? kExpandWarps : 1);  // packed: the expand warps publish the int8 stage
       mbar_init(&empty_bar[s], 1);
+      if (kPacked) {
+        mbar_init(&raw_full[s], 1);
+        mbar_init(&raw_empty[s], kExpandWarps);
+      }
     }
     for (int r = 0; r < 2; ++r) {
       mbar_init(&acc_full[r], 1);
@@ -89,6 +99,20 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
         for (int t = it.t0; t < it.t1; t += it.bk, ++iter) {
           if ((iter & 1) != pw) {
+            if (++stage == p.stages) { stage = 0; phase ^= 1; }
+            continue;
+          }
+          if (kPacked) {
+            // packed boxes {64 B, bk rows} land in the raw ring; the expand warps own the int8 ring
+            mbar_wait(&raw_empty[stage], phase ^ 1);
+            const uint32_t raw_panel = static_cast<uint32_t>(it.bk) * (kPanelBytes / 2);
+            mbar_expect_tx(&raw_full[stage], raw_panel * it.n_load);
+            uint8_t *rdst = raw + static_cast<size_t>(stage) * raw_stage_bytes;
+            for (int l = 0; l < it.n_load; ++l) {
+              const bool is_a = l >= it.nblk_load;
+              const int x = (is_a ? it.xa : it.x0 + l * it.dx) >> 1;  // one byte per sample: half the offset
+              tma_load_2d(rdst + l * raw_panel, map, &raw_full[stage], x, t, pol);
+            }
             if (++stage == p.stages) { stage = 0; phase ^= 1; }
             continue;
           }
@@ -190,11 +214,61 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
         ring += n_chunks;
       }
     }
+  } else if (kPacked && warp >= kExpandWarp0) {
+    // ===================================================================== expand warps (4-bit input)
+    // raw ring -> int8 ring: each byte (low nibble Re, high nibble Im, two's complement, DESIGN
+    // reading R18) becomes the int8 pair (16 Re, 16 Im), written in the MN-major 128-byte-swizzled operand
+    // layout the TMA would have produced for int8 input.  A nibble moved to the top of its byte IS 16 x its
+    // two's-complement value, so no sign extension is needed: the Gram sums come out 256 x too large, exactly,
+    // and the epilogue shifts them right by 8 (p.out_shift).  |256 V| <= T * 2 * 128^2 still fits int32.
+    const int et = threadIdx.x - kExpandWarp0 * 32;  // 0 .. 127
+    int stage = 0;
+    uint32_t phase = 0;
+    I8Iter cur = iter_init(p);
+    for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
+      if (!iter_valid(p, cur)) continue;
+      const I8Item it = decode_item(p, cur, rank);
+      const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
+      const int n_chunks = it.n_load * it.bk * 4;  // 16-byte packed chunks of this stage
+      const int sh = 31 - __clz(it.bk * 4);
+      for (int t = it.t0; t < it.t1; t += it.bk) {
+        mbar_wait(&raw_full[stage], phase);       // packed bytes have landed
+        mbar_wait(&empty_bar[stage], phase ^ 1);  // the int8 slot has been consumed by the MMAs
+        const uint8_t *src = raw + static_cast<size_t>(stage) * raw_stage_bytes;
+        uint8_t *dst = smem + static_cast<size_t>(stage) * p.stage_bytes;
+        for (int idx = et; idx < n_chunks; idx += kExpandWarps * 32) {
+          const int l = idx >> sh;            // panel (bk * 4 chunks each, a power of two)
+          const int rem = idx & ((1 << sh) - 1);
+          const int k = rem >> 2, q = rem & 3;
+          const uint4 w = *reinterpret_cast<const uint4 *>(src + l * (panel_bytes / 2) + k * 64 + q * 16);
+          const uint32_t in[4] = {w.x, w.y, w.z, w.w};
+          uint32_t out[8];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const uint32_t re = (in[u] << 4) & 0xF0F0F0F0u;  // 16 * Re in every byte
+            const uint32_t im = in[u] & 0xF0F0F0F0u;         // 16 * Im in every byte
+            out[2 * u] = __byte_perm(re, im, 0x5140);      // re0 im0 re1 im1
+            out[2 * u + 1] = __byte_perm(re, im, 0x7362);  // re2 im2 re3 im3
+          }
+          uint8_t *row = dst + l * panel_bytes + k * kPanelBytes;
+          const int sw = k & 7;  // 128-byte swizzle: 16-byte chunk index XOR (row mod 8)
+          *reinterpret_cast<uint4 *>(row + (((2 * q) ^ sw) << 4)) = make_uint4(out[0], out[1], out[2], out[3]);
+          *reinterpret_cast<uint4 *>(row + (((2 * q + 1) ^ sw) << 4)) = make_uint4(out[4], out[5], out[6], out[7]);
+        }
+        fence_proxy_async();  // generic-proxy writes -> visible to the tensor core's (async-proxy) reads
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(&full_bar[stage]);
+          mbar_arrive(&raw_empty[stage]);
+        }
+        if (++stage == p.stages) { stage = 0; phase ^= 1; }
+      }
+    }
   } else if (warp < kEpiWarps && !(probe & 4)) {
     // ===================================================================== epilogue
     const int ew = warp & 3;         // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
-    i8_epilogue(p, tmem_base, smem + static_cast<size_t>(p.stages) * p.stage_bytes + warp * kEpiWarpBytes,
+    i8_epilogue(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
                 acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 
@@ -211,6 +285,13 @@ xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_cons
                   const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
   if (p.probe) xengine_i8_body<false, true>(tmap256, tmap128, tmap64, p);
   else         xengine_i8_body<false, false>(tmap256, tmap128, tmap64, p);
+}
+
+// 4-bit packed input (the paper's "1-byte mode"): 16 warps, the last four expand nibbles to int8.
+__global__ void __launch_bounds__(kI4Threads, 1)
+xengine_i4_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
+                  const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
+  xengine_i8_body<false, false, true>(tmap256, tmap128, tmap64, p);
 }
 
 // CTA pairs: tcgen05.mma.cta_group::2, M = 256 (one 128-row panel per CTA), each CTA stages half of B.
