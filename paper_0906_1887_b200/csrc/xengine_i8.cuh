@@ -32,8 +32,8 @@ namespace corr {
 
 constexpr int kI8Threads = 384;    // 4 control warps + 8 epilogue warps
 constexpr int kEpiWarps = 8;
-constexpr int kExpandWarp0 = 12, kExpandWarps = 4;  // 4-bit input only (512-thread launch)
-constexpr int kI4Threads = 512;
+constexpr int kExpandWarp0 = 12, kExpandWarps = 8;  // 4-bit input only (640-thread launch)
+constexpr int kI4Threads = 640;
 constexpr int kProducerWarp = 8, kMmaWarp = 9, kAllocWarp = 10, kProducerWarp2 = 11;
 constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64 complex int8 samples
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
