@@ -98,6 +98,21 @@ int corr_launches_per_call(const corr_handle *h);
 int corr_set_turn(corr_handle *h, int mode);
 
 /*
+ * corr_set_accumulate -- accumulate mode (each batch's products are ADDED to the
+ * accumulators).  on != 0: corr_xengine adds the sums of its integration to d_vis instead of overwriting
+ * it (the caller zeroes d_vis before the first call; integer sums stay exact as long as they fit int32).
+ */
+int corr_set_accumulate(corr_handle *h, int on);
+
+/*
+ * corr_normalize -- read-out (the accumulators are "divided by the number of times they were
+ * updated"): d_out[c][b] = d_vis[c][b] / count as (float re, float im); d_vis holds int32 pairs (CI8, CI4)
+ * or float pairs (CF32).  d_out has corr_vis_bytes(h) bytes, 16-byte aligned, may not alias d_vis unless the
+ * dtype is CF32.  Asynchronous on `stream`.
+ */
+int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out, void *stream);
+
+/*
  * corr_set_probe -- DIAGNOSTICS ONLY (results are garbage while a probe is on): switches engines of the CI8
  * kernel off so that the others can be timed alone.  Bit mask: 1 = skip the MMAs, 2 = skip the TMA loads
  * (producer only hand-shakes), 4 = no epilogue, 8 = no producer and no stage hand-shake at all, 16 = epilogue

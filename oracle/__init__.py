@@ -48,6 +48,9 @@ def _load():
         _lib.oracle_xengine_ci4.argtypes = [P, L, L, L, L, L, P, I]
         _lib.oracle_unpack_ci4.argtypes = [ctypes.c_ubyte, ctypes.POINTER(I), ctypes.POINTER(I)]
         _lib.oracle_unpack_ci4.restype = None
+        _lib.oracle_readout_i32.argtypes = [P, L, ctypes.c_double, P]
+        _lib.oracle_readout_f64.argtypes = [P, L, ctypes.c_double, P]
+        _lib.oracle_readout_i32.restype = _lib.oracle_readout_f64.restype = None
         _lib.oracle_full_matrix_ci8.argtypes = [P, L, L, L, L, P]
         _lib.oracle_full_matrix_cf32.argtypes = [P, L, L, L, L, P]
         _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
@@ -98,6 +101,19 @@ def xengine_ci4(x, c_begin=0, c_end=None, threads=1):
     if rc != 0:
         raise MemoryError("oracle allocation failed")
     return vis
+
+
+def readout(vis, count):
+    """Time-averaged visibilities: raw sums / number of accumulated samples -> float64."""
+    vis = np.ascontiguousarray(vis)
+    out = np.empty(vis.shape, dtype=np.float64)
+    if vis.dtype == np.int32:
+        _load().oracle_readout_i32(vis.ctypes.data, vis.size, float(count), out.ctypes.data)
+    elif vis.dtype == np.float64:
+        _load().oracle_readout_f64(vis.ctypes.data, vis.size, float(count), out.ctypes.data)
+    else:
+        raise ValueError("readout expects int32 or float64 sums")
+    return out
 
 
 def xengine_cf32(x, c_begin=0, c_end=None, threads=1):

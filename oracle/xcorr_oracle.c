@@ -247,3 +247,16 @@ int oracle_xengine_ci4(const uint8_t *x, long n_time, long n_chan, long n_inputs
     }
     return status;
 }
+
+/*
+ * Read-out (Fig. 1 caption): "the accumulators are ... divided by the number of times they
+ * were updated" -> the time-averaged visibility.  Plain division in float64.
+ */
+void oracle_readout_i32(const int32_t *vis, long n_scalars, double count, double *out)
+{
+    for (long k = 0; k < n_scalars; ++k) out[k] = (double)vis[k] / count;
+}
+void oracle_readout_f64(const double *vis, long n_scalars, double count, double *out)
+{
+    for (long k = 0; k < n_scalars; ++k) out[k] = vis[k] / count;
+}

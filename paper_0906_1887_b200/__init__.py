@@ -18,7 +18,7 @@ CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
-           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma")
+           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize")
 
 _lib = None
 
@@ -48,6 +48,9 @@ def lib():
         L.corr_launches_per_call.restype, L.corr_launches_per_call.argtypes = ci, [vp]
         L.corr_set_turn.restype, L.corr_set_turn.argtypes = ci, [vp, ci]
         L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
+        L.corr_set_accumulate.restype, L.corr_set_accumulate.argtypes = ci, [vp, ci]
+        L.corr_normalize.restype = ci
+        L.corr_normalize.argtypes = [vp, vp, ctypes.c_double, vp, vp]
         L.corr_probe_mma.restype = ci
         L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
@@ -97,6 +100,21 @@ class Correlator:
     def set_turn(self, mode):
         if lib().corr_set_turn(self._h, mode) != CORR_OK:
             _raise()
+
+    # -- corr_set_accumulate / corr_normalize
+    def set_accumulate(self, on=True):
+        if lib().corr_set_accumulate(self._h, 1 if on else 0) != CORR_OK:
+            _raise()
+
+    def normalize(self, d_vis, count, d_out=None, stream=None):
+        """d_vis (raw sums) / count -> float32 [C][N(N+1)/2][2] (PAPER.md:84 read-out)."""
+        import torch
+        if d_out is None:
+            d_out = torch.empty(d_vis.shape, dtype=torch.float32, device="cuda")
+        rc = lib().corr_normalize(self._h, d_vis.data_ptr(), float(count), d_out.data_ptr(), _stream_ptr(stream))
+        if rc != CORR_OK:
+            _raise()
+        return d_out
 
     def empty_vis(self, n=1):
         import torch

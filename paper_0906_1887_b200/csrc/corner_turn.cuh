@@ -48,4 +48,28 @@ __global__ void __launch_bounds__(kTurnThreads) corner_turn_kernel(const TurnPar
   }
 }
 
+// Read-out normalisation ("accumulators are ... divided by the number of times they were
+// updated"): out[k] = vis[k] / count, int32 or float sums -> float.  One pass, 16-byte vectors.
+struct NormParams {
+  const void *vis;
+  float *out;
+  long long n;     // scalars (2 per visibility); a multiple of 4
+  float inv_count;
+  int is_int;
+};
+__global__ void __launch_bounds__(256) normalize_kernel(const NormParams p) {
+  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  for (long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; k < p.n / 4; k += stride) {
+    float4 o;
+    if (p.is_int) {
+      const int4 v = reinterpret_cast<const int4 *>(p.vis)[k];
+      o = make_float4(v.x * p.inv_count, v.y * p.inv_count, v.z * p.inv_count, v.w * p.inv_count);
+    } else {
+      const float4 v = reinterpret_cast<const float4 *>(p.vis)[k];
+      o = make_float4(v.x * p.inv_count, v.y * p.inv_count, v.z * p.inv_count, v.w * p.inv_count);
+    }
+    reinterpret_cast<float4 *>(p.out)[k] = o;
+  }
+}
+
 }  // namespace corr

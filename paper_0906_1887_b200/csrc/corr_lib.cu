@@ -69,6 +69,7 @@ struct corr_handle {
   int n_sms;
   int turn_mode;
   int probe;
+  int accumulate;
   // CI8 plan
   int pair_mode, grid_i8, use_pairs;
   size_t smem_i8;
@@ -277,6 +278,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->n_sms = prop.multiProcessorCount;
   h->turn_mode = CORR_TURN_FUSED;
   h->probe = 0;
+  h->accumulate = 0;
   h->d_items_f32 = nullptr;
   h->d_scratch = nullptr;
   h->d_stream_in[0] = h->d_stream_in[1] = nullptr;
@@ -370,6 +372,30 @@ int corr_set_probe(corr_handle *h, int mode) {
   return CORR_OK;
 }
 
+int corr_set_accumulate(corr_handle *h, int on) {
+  if (!h) return fail(CORR_EINVAL, "corr_set_accumulate: NULL handle");
+  h->accumulate = on ? 1 : 0;
+  return CORR_OK;
+}
+
+int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out, void *stream) {
+  if (!h || !d_vis || !d_out) return fail(CORR_EINVAL, "corr_normalize: NULL argument");
+  if (!(count > 0)) return fail(CORR_EINVAL, "corr_normalize: count must be positive");
+  if ((reinterpret_cast<uintptr_t>(d_vis) | reinterpret_cast<uintptr_t>(d_out)) & 15)
+    return fail(CORR_EINVAL, "corr_normalize: pointers must be 16-byte aligned");
+  corr::NormParams np;
+  np.vis = d_vis;
+  np.out = static_cast<float *>(d_out);
+  np.n = static_cast<long long>(h->vis_bytes / 4);
+  np.inv_count = static_cast<float>(1.0 / count);
+  np.is_int = h->dtype != CORR_CF32;
+  if (np.n % 4) return fail(CORR_EUNSUPPORTED, "corr_normalize: odd number of visibilities");
+  const int blocks = static_cast<int>(std::min<long long>((np.n / 4 + 255) / 256, 148 * 8));
+  corr::normalize_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(np);
+  CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
 int corr_set_turn(corr_handle *h, int mode) {
   if (!h) return fail(CORR_EINVAL, "corr_set_turn: NULL handle");
   if (h->dtype != CORR_CI8) return fail(CORR_EUNSUPPORTED, "corr_set_turn: only the CI8 path has two corner-turn realisations");
@@ -434,6 +460,7 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     fp.n_chan = h->n_chan;
     fp.n_inputs = h->n_inputs;
     fp.n_baselines = h->n_baselines;
+    fp.accumulate = h->accumulate;
     corr::xengine_f32_kernel<<<h->n_items_f32, h->f32_threads, 0, st>>>(fp);
     CUDA_TRY(cudaGetLastError());
     return CORR_OK;
@@ -453,7 +480,8 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.vis = static_cast<int2 *>(d_vis);
   ip.probe = h->probe;
   ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
-  if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
+  ip.accumulate = h->accumulate;
+  if (ip.n_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
   if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<h->grid_i8, corr::kI4Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   else if (ip.pair2) corr::xengine_i8_pair_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
   else          corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);

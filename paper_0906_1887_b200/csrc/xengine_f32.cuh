@@ -27,6 +27,7 @@ struct F32Params {
   int n_items;
   int n_time, n_chan, n_inputs;
   long long n_baselines;
+  int accumulate;  // 1: d_vis += this integration; every element has exactly one writer
 };
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
@@ -137,7 +138,11 @@ __global__ void __launch_bounds__(kF32Threads) xengine_f32_kernel(const F32Param
 #pragma unroll
       for (int b = 0; b < 4; ++b) {
         const int j = J * kF32Block + 4 * tj + b;
-        if (j <= i) row[j] = make_float2(re[a][b], j == i ? 0.f : im[a][b]);
+        if (j <= i) {
+          float2 v = make_float2(re[a][b], j == i ? 0.f : im[a][b]);
+          if (p.accumulate) { const float2 old = row[j]; v.x += old.x; v.y += old.y; }
+          row[j] = v;
+        }
       }
     }
   }

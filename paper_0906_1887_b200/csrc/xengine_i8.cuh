@@ -60,6 +60,7 @@ struct I8Params {
   int turned;        // 0: d_in is [T][C][2N] (2-D maps); 1: scratch is [G][T][W] (3-D maps)
   int probe;         // diagnostics only (corr_set_probe)
   int out_shift;     // 8 for 4-bit input (operands are 16 x the samples), else 0
+  int accumulate;    // 1: add this integration into d_vis instead of overwriting it
   long long n_baselines;
   int2 *vis;
   unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11; pair: Ip | (J0 / 2) << 6 | wide << 11

@@ -23,7 +23,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
                                             int hsel, int lane, int rank, bool pair, int probe) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
-  const bool atomic = p.n_slices > 1;
+  const bool atomic = p.n_slices > 1 || p.accumulate;  // reduce-add into d_vis instead of plain stores
   const int out_shift = p.out_shift;
   int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kEpiRowBytes / 4) + part;
   uint32_t ring = 0;

@@ -52,3 +52,22 @@ def test_p12_matches_the_int8_oracle_on_unpacked_data():
     assert np.array_equal(back, x)
     assert np.array_equal(oracle.xengine_ci4(p, threads=2), oracle.xengine_ci8(x))
     assert np.array_equal(oracle.xengine_ci4(p, 1, 3), oracle.xengine_ci8(x, 1, 3))
+
+
+def test_p13_readout_is_the_time_average():
+    """PAPER.md:84: sums divided by the update count.  Constant input x_i: the average is x_i conj(x_j) exactly;
+    and accumulating two batches equals one long integration (pin P4), so count = T1 + T2."""
+    T1, T2, N = 40, 24, 4
+    vals = np.array([[3, -2], [1, 1], [-7, 0], [0, 5]], np.int8)
+    x = np.broadcast_to(vals, (T1 + T2, 1, N, 2)).copy()
+    total = oracle.xengine_ci8(x[:T1]).astype(np.int64) + oracle.xengine_ci8(x[T1:]).astype(np.int64)
+    assert np.array_equal(total, oracle.xengine_ci8(x))
+    avg = oracle.readout(oracle.xengine_ci8(x), T1 + T2)
+    b = 0
+    for i in range(N):
+        for j in range(i + 1):
+            z = complex(*vals[i].tolist()) * complex(*vals[j].tolist()).conjugate()
+            assert avg[0, b, 0] == z.real and avg[0, b, 1] == z.imag
+            b += 1
+    f = oracle.readout(np.array([[[1.5, -3.0]]]), 4)
+    assert f[0, 0, 0] == 0.375 and f[0, 0, 1] == -0.75
