@@ -26,6 +26,17 @@ def test_roofline_times_match_survey_table():
     assert w.cmacs == 10000 * 768 * 2080 and w.in_bytes == 983040000 and w.vis_bytes == 12779520
 
 
+def test_channel_sharding_covers_every_channel_once():
+    sys.path.insert(0, ROOT)
+    import bench
+    for n_chan, world in [(768, 8), (768, 5), (128, 3), (7, 8), (1536, 2)]:
+        ranges = [bench.shard_channels(n_chan, world, r) for r in range(world)]
+        assert ranges[0][0] == 0 and ranges[-1][1] == n_chan
+        assert all(a[1] == b[0] for a, b in zip(ranges, ranges[1:]))
+        sizes = [b - a for a, b in ranges]
+        assert max(sizes) - min(sizes) <= 1
+
+
 def test_reference_arm_prints_contract_line():
     env = dict(os.environ, OMP_NUM_THREADS="2")
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "c1",
