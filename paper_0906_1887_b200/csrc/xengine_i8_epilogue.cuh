@@ -16,16 +16,24 @@
 namespace corr {
 
 constexpr int kEpiRowBytes = 272;  // 32 complex int32 + one alignment slot, 16-byte multiple
+constexpr int kEpiRowBytesPlain = 264;  // plain-store path: 66-word stride, conflict-free staging writes
 constexpr int kEpiWarpBytes = 16 * kEpiRowBytes;  // 4224 B per epilogue warp
 
+// kAtomic: reduce-add into d_vis (time-sliced or accumulating items) instead of plain stores.  kShift: 8 for
+// 4-bit input (operands are 16 x the samples), else 0.  Both are compile-time so that the plain-store path is
+// the bare minimum per value: one SHFL, one IMAD (v + sgn * partner), one conflict-free STS.
+template <bool kAtomic, int kShift>
 __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_base, uint8_t *stage_buf,
                                             uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
                                             int hsel, int lane, int rank, bool pair, int probe) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
-  const bool atomic = p.n_slices > 1 || p.accumulate;  // reduce-add into d_vis instead of plain stores
-  const int out_shift = p.out_shift;
-  int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kEpiRowBytes / 4) + part;
+  constexpr bool atomic = kAtomic;
+  const int sgn = part ? -1 : 1;  // Re = G[2i][2j] + G[2i+1][2j+1], Im = G[2i+1][2j] - G[2i][2j+1]
+  // staging row stride: 272 B keeps rows 16-byte aligned for the bulk reduce-add; 264 B (66 words) makes the
+  // 4-byte staging writes of the 32 lanes hit 32 different banks on the plain-store path
+  constexpr int kRowB = kAtomic ? kEpiRowBytes : kEpiRowBytesPlain;
+  int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kRowB / 4) + part;
   uint32_t ring = 0;
   I8Iter cur = iter_init(p);
   for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
@@ -83,12 +91,11 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
           for (int jj = 0; jj < 16; ++jj) {
             const int o0 = __shfl_xor_sync(0xffffffffu, static_cast<int>(v0[2 * jj + 1]), 1);
             const int o1 = __shfl_xor_sync(0xffffffffu, static_cast<int>(v1[2 * jj + 1]), 1);
-            int a0 = part ? (static_cast<int>(v0[2 * jj]) - o0) : (static_cast<int>(v0[2 * jj]) + o0);
-            int a1 = part ? (static_cast<int>(v1[2 * jj]) - o1) : (static_cast<int>(v1[2 * jj]) + o1);
-            a0 >>= out_shift;  // 4-bit input: sums are exact multiples of 256
-            a1 >>= out_shift;
-            if (part && (j0 + jj) == i_row) a0 = 0;       // Im of an autocorrelation is exactly 0
-            if (part && (j0 + 16 + jj) == i_row) a1 = 0;
+            int a0 = o0 * sgn + static_cast<int>(v0[2 * jj]);
+            int a1 = o1 * sgn + static_cast<int>(v1[2 * jj]);
+            if (kShift) { a0 >>= kShift; a1 >>= kShift; }  // 4-bit input: sums are exact multiples of 256
+            // (Im of an autocorrelation needs no special case: G is computed in exact integers and is
+            //  symmetric, so G[2i+1][2i] - G[2i][2i+1] is exactly 0)
             st_row[jj * 2] = a0;                          // even lane: Re -> .x, odd lane: Im -> .y
             st_row[(16 + jj) * 2] = a1;
           }
@@ -102,7 +109,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
               if (cnt > 0) {
                 const long long e0 = static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j0;
                 const int sh = static_cast<int>(e0 & 1);
-                const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kEpiRowBytes) + sh;  // element 0
+                const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kRowB) + sh;  // element 0
                 int2 *grow = p.vis + e0;
                 int head = sh;                         // one leading element if e0 is odd
                 int body = (cnt - head) & ~1;          // aligned pairs
@@ -125,22 +132,27 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
             }
 
           } else if (!(probe & 16)) {
-            // one packed-triangle row per instruction: 32 lanes x 8 B = 256 contiguous bytes
+            // one packed-triangle row per instruction: 32 lanes x 8 B = 256 contiguous bytes.  N_I is a multiple
+            // of 32, so every row and column of the half block exists; only diagonal blocks need the j <= i test.
             const int j = j0 + lane;
-            int i = i0_w;
+            const int i = i0_w;
             int2 *row = p.vis + (static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j);
             const int2 *src = reinterpret_cast<const int2 *>(stage_buf) + lane;
             int2 val[16];
 #pragma unroll
-            for (int rr = 0; rr < 16; ++rr) val[rr] = src[rr * (kEpiRowBytes / 8)];  // 16 independent loads
+            for (int rr = 0; rr < 16; ++rr) val[rr] = src[rr * (kRowB / 8)];  // 16 independent loads
+            if (!diag_blk) {
 #pragma unroll
-            for (int rr = 0; rr < 16; ++rr) {
-              if (i < p.n_inputs && j <= i && j < p.n_inputs) {
-                if (atomic) put_vis<true>(row, val[rr].x, val[rr].y);
-                else        put_vis<false>(row, val[rr].x, val[rr].y);
+              for (int rr = 0; rr < 16; ++rr) {
+                *row = val[rr];
+                row += i + rr + 1;  // next row of the triangle starts i+1 elements further on
               }
-              ++i;
-              row += i;  // next row of the triangle starts i+1 elements further on
+            } else {
+#pragma unroll
+              for (int rr = 0; rr < 16; ++rr) {
+                if (j <= i + rr) *row = val[rr];
+                row += i + rr + 1;
+              }
             }
           }
           __syncwarp();

@@ -268,8 +268,13 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     // ===================================================================== epilogue
     const int ew = warp & 3;         // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
-    i8_epilogue(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
-                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+    constexpr int kShift = kPacked ? 8 : 0;
+    if (p.n_slices > 1 || p.accumulate)
+      i8_epilogue<true, kShift>(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+    else
+      i8_epilogue<false, kShift>(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                             acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 
   tc_fence_before();
