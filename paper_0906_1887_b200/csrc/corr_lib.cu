@@ -100,25 +100,50 @@ void plan_i8(corr_handle *h) {
   int max_load = 1;
   if (ip.diag) {
     ip.n_panels = h->pair_mode ? (C + 1) / 2 : C;
-    ip.n_groups = (ip.n_panels + 3) / 4;
-    ip.n_kinds = 1;
-    max_load = 4;
-    // split the integration into time slices until the grid is filled evenly
-    const int base = ip.n_groups, G = h->n_sms;
-    int best_s = 1;
-    double best_eff = 0.0;
-    for (int s = 1; s <= 64; ++s) {
-      int len = ((T + s - 1) / s + 63) / 64 * 64;
-      if (len < 128 && s > 1) break;
-      const int s_eff = (T + len - 1) / len;
-      if (s_eff != s) continue;
-      const long long n = 1LL * base * s;
-      const long long rounds = (n + G - 1) / G;
-      // load of the busiest CTA in units of samples vs the mean
-      const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
-      if (eff > best_eff + 0.02) { best_eff = eff; best_s = s; }
-      if (best_eff >= 0.95) break;
+    // Items are the diagonal blocks of `gsize` ADJACENT panels over one time slice.  Large inputs: gsize = 4
+    // (512-byte HBM runs) and as many time slices as fill the grid evenly (slices accumulate with reduce-add
+    // into a zeroed d_vis).  Small inputs (<= 64 MB) are latency-bound: the zeroing node, the reduce-adds and
+    // their completion waits cost more than the load itself, so the plan with the least modelled time is
+    // taken, which usually is whole integrations (no slices) of 1 or 2 panels spread over more SMs.
+    const int G = h->n_sms;
+    int best_g = 4, best_s = 1;
+    double best_t = 1e30;
+    const bool small = h->in_bytes <= (64u << 20);
+    for (int g = 4; g >= (small ? 1 : 4); g >>= 1) {
+      const int base = (ip.n_panels + g - 1) / g;
+      int cand_s = 1;
+      double cand_eff = 0.0;
+      for (int s = 1; s <= 64; ++s) {
+        int len = ((T + s - 1) / s + 63) / 64 * 64;
+        if (len < 128 && s > 1) break;
+        const int s_eff = (T + len - 1) / len;
+        if (s_eff != s) continue;
+        const long long n = 1LL * base * s;
+        const long long rounds = (n + G - 1) / G;
+        // load of the busiest CTA in units of samples vs the mean
+        const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
+        if (small) {
+          // modelled time: rounds x (item bytes at ~80 GB/s per SM) + the fixed cost of a sliced launch
+          const double t = 1e-9 * rounds * (1.0 * g * 128 * std::min(len, T)) / 80.0 + (s > 1 ? 4e-6 : 0.0);
+          if (t < best_t - 1e-7) { best_t = t; best_g = g; best_s = s; }
+        } else {
+          if (eff > cand_eff + 0.02) { cand_eff = eff; cand_s = s; }
+          if (cand_eff >= 0.95) break;
+        }
+      }
+      if (!small) best_s = cand_s;
     }
+    if (const char *ov = getenv("CORR_DIAG_PLAN")) {  // tests / experiments: "gsize,slices"
+      int g = 0, sl = 0;
+      if (sscanf(ov, "%d,%d", &g, &sl) == 2 && (g == 1 || g == 2 || g == 4) && sl >= 1 && sl <= 64) {
+        const int len = ((T + sl - 1) / sl + 63) / 64 * 64;
+        if (sl == 1 || (len >= 128 && (T + len - 1) / len == sl)) { best_g = g; best_s = sl; }
+      }
+    }
+    ip.gsize = best_g;
+    ip.n_groups = (ip.n_panels + best_g - 1) / best_g;
+    ip.n_kinds = 1;
+    max_load = best_g;
     ip.n_slices = best_s;
     ip.slice_len = best_s == 1 ? T : ((T + best_s - 1) / best_s + 63) / 64 * 64;
   } else {
@@ -127,8 +152,9 @@ void plan_i8(corr_handle *h) {
     int k = 0;
     // CTA pairs (cta_group::2) from N_I = 512 up; already from N_I = 256 when the integration is long
     // enough (T >= 2048) for 512-wide tiles, whose epilogue cannot overlap the next tile's MMAs
-    const bool wide_ok = T >= 2048 && panels_per_chan >= 4;
-    if (h->use_pairs && (panels_per_chan >= 8 || wide_ok)) {
+    const bool long_ok = T >= 2048 && panels_per_chan >= 4;
+    const bool wide_ok = long_ok && !getenv("CORR_NO_WIDE");
+    if (h->use_pairs && (panels_per_chan >= 8 || long_ok)) {
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;
       max_load = 2;

@@ -42,7 +42,8 @@ constexpr int kMaxKinds = 1056;   // slab kinds per channel at N_I = 4096 (64 pa
 
 struct I8Params {
   // ---- schedule (uniform) ----
-  int n_groups;      // diag: groups of 4 panels; slab: channels
+  int n_groups;      // diag: groups of gsize panels; slab: channels
+  int gsize;         // diag: adjacent panels per item (4, or 2 / 1 for small problems)
   int n_kinds;       // items per group (diag: 1)
   int n_slices;      // time slices per integration (> 1 => results are accumulated with red.add)
   int slice_len;     // samples per slice (multiple of 256 when n_slices > 1)
@@ -117,8 +118,8 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
   it.t1 = min(p.n_time, it.t0 + p.slice_len);
   const int row = 2 * p.n_inputs;  // bytes per (t, c)
   if (p.diag) {
-    const int panel0 = grp * 4;
-    it.nblk = min(4, p.n_panels - panel0);
+    const int panel0 = grp * p.gsize;
+    it.nblk = min(p.gsize, p.n_panels - panel0);
     it.n_load = it.nblk;
     it.a_slot = 0;
     it.chan = 0; it.I = 0; it.J0 = panel0;

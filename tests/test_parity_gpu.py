@@ -213,3 +213,14 @@ def test_mma_probe_runs_at_the_tensor_rate(pkg):
     r = pkg.probe_mma(128, 256, True, 8192, random_fill=True)
     assert 120.0 <= r["cycles_per_mma"] <= 150.0, r
     assert r["tops"] > 3000.0, r
+
+
+# Every plan of the diag schedule (N_I <= 64): gsize adjacent panels per item x time slices.  Small inputs
+# default to whole integrations of 1-2 panels; "4,s" is what the large configs (c2) run, incl. the reduce-add path.
+@pytest.mark.parametrize("plan", ["4,1", "4,3", "2,1", "2,2", "1,1", "1,4"])
+@pytest.mark.parametrize("N,C,T", [(64, 11, 700), (32, 13, 530), (64, 1, 129)])
+def test_ci8_diag_plans_bit_exact(pkg, monkeypatch, plan, N, C, T):
+    monkeypatch.setenv("CORR_DIAG_PLAN", plan)
+    w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
