@@ -7,7 +7,8 @@ package.  The product package never does (tests/test_independence.py checks).
 All arithmetic is in ``xcorr_oracle.c`` (read its header for the passages it
 follows: PAPER.md:47, :53, :84, :107, :115).  This file only marshals numpy
 arrays.  Parity status: every function below is pinned by
-``tests/test_oracle_pins.py`` (P1-P9, P11-P12 for the 4-bit mode, tests/golden/); none is "parity unpinned".
+``tests/test_oracle_pins.py`` (P1-P9, P11-P12 for the 4-bit mode, tests/golden/) or, for the F-stage
+(``fstage_oracle.c``), ``tests/test_oracle_fstage_pins.py`` (F1-F7); none is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -19,6 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "xcorr_oracle.c")
+_SRC_F = os.path.join(_HERE, "fstage_oracle.c")  # F-stage (unpack + DFT), SURVEY 8(f) row 3
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
@@ -29,11 +31,11 @@ class OracleOverflow(ArithmeticError):
 
 def build(force: bool = False) -> str:
     """gcc -O2, no fused multiply-add contraction (Im V_ii must be exactly 0 in float64)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_F)):
         tmp = f"{_LIB}.{os.getpid()}.tmp"
         subprocess.check_call(
             ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-             "-o", tmp, _SRC])
+             "-o", tmp, _SRC, _SRC_F, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -55,6 +57,8 @@ def _load():
         _lib.oracle_full_matrix_cf32.argtypes = [P, L, L, L, L, P]
         _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
         _lib.oracle_one_visibility_cf32.argtypes = [P, L, L, L, L, L, L, P]
+        _lib.oracle_fstage_ci8.argtypes = [P, L, L, L, P, I]
+        _lib.oracle_xengine_cf64.argtypes = [P, L, L, L, P, I]
     return _lib
 
 
@@ -155,3 +159,28 @@ def one_visibility_cf32(x, c, i, j):
     out = np.empty(2, dtype=np.float64)
     _load().oracle_one_visibility_cf32(x.ctypes.data, T, C, N, c, i, j, out.ctypes.data)
     return float(out[0]), float(out[1])
+
+
+# --------------------------------------------------------------------------- F-stage (fstage_oracle.c)
+
+def fstage_ci8(x, threads=1):
+    """x: [B][N_C][N_I][2] int8 raw voltages -> [B][N_C][N_I][2] float64 spectra, the plain O(N^2) DFT with
+    exp(-2 pi i k n / N), unnormalised (readings R19-R21)."""
+    x = np.ascontiguousarray(x)
+    assert x.dtype == np.int8 and x.ndim == 4 and x.shape[3] == 2, x.shape
+    B, N, I, _ = x.shape
+    out = np.empty((B, N, I, 2), dtype=np.float64)
+    rc = _load().oracle_fstage_ci8(x.ctypes.data, B, N, I, out.ctypes.data, int(threads))
+    assert rc == 0
+    return out
+
+
+def xengine_cf64(x, threads=1):
+    """x: [T][C][N][2] float64 spectra -> [C][N(N+1)/2][2] float64 (the X-engine definition in float64)."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    assert x.ndim == 4 and x.shape[3] == 2, x.shape
+    T, C, N, _ = x.shape
+    vis = np.empty((C, N * (N + 1) // 2, 2), dtype=np.float64)
+    rc = _load().oracle_xengine_cf64(x.ctypes.data, T, C, N, vis.ctypes.data, int(threads))
+    assert rc == 0
+    return vis
