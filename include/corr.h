@@ -153,6 +153,36 @@ int corr_corner_turn(corr_handle *h, const void *d_in, void *d_out, void *stream
 int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
                     void *d_vis, double *stats);
 
+/* ------------------------------------------------------------------------------------------------
+ * F-stage: the two steps in front of the CMAC in the paper's correlator,
+ *   "1- unpacking a block of data, which involves reordering samples ... 2- Fourier transforming into
+ *    frequency space"
+ *   "taking a block of N_I x N_C complex samples which are ordered with input varying most quickly,
+ *    converting to floating-point format and putting the samples into N_I arrays of length N_C"
+ *
+ *   "the FFT is N_C channels in input and output"
+ *
+ *   X[b][k][i] = sum_{n=0}^{N_C-1} x[b][n][i] * exp(-2 pi i k n / N_C)
+ *
+ * forward sign, unnormalised, natural channel order k = 0 (DC) first (readings R19, R20).
+ *   d_raw  : device, [n_batch][n_fft][n_inputs] complex int8 (int8 re, int8 im; any 5+5-bit sample of
+ *            PAPER.md:69 is one; reading R21), input index fastest; 16-byte aligned; read only.
+ *   d_spec : device, [n_batch][n_fft][n_inputs] (float re, float im), overwritten; 16-byte aligned; must
+ *            not alias d_raw.  With n_batch = n_time * n_bands this IS corr_xengine's CF32 input
+ *            [n_time][n_chan = n_bands * n_fft][n_inputs].
+ * corr_fstage_create: n_fft must be 128 (the paper's N_C), n_inputs a multiple of 32 and
+ * <= 4096, n_batch >= 1; NULL + corr_last_error() otherwise (CORR_EINVAL / CORR_EUNSUPPORTED / CORR_EARCH /
+ * CORR_ECUDA / CORR_EALLOC).  corr_fstage_run is asynchronous on `stream`; returns CORR_OK, CORR_EINVAL or
+ * CORR_ECUDA.  FP32 arithmetic: |dX| <= 1e-5 * ||x[b][:][i]||_2 per channel against the float64 definition
+ * (DESIGN.md section 6).  The handle owns nothing on the device; corr_fstage_destroy(NULL) is a no-op.
+ */
+typedef struct corr_fstage corr_fstage; /* opaque */
+corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch);
+int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *stream);
+int corr_fstage_destroy(corr_fstage *f);
+size_t corr_fstage_in_bytes(const corr_fstage *f);  /* n_batch * n_fft * n_inputs * 2 */
+size_t corr_fstage_out_bytes(const corr_fstage *f); /* n_batch * n_fft * n_inputs * 8 */
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,7 +18,8 @@ CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
-           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize")
+           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize",
+           "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes")
 
 _lib = None
 
@@ -54,6 +55,11 @@ def lib():
         L.corr_probe_mma.restype = ci
         L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
+        L.corr_fstage_create.restype, L.corr_fstage_create.argtypes = vp, [ci, ci, ci]
+        L.corr_fstage_run.restype, L.corr_fstage_run.argtypes = ci, [vp, vp, vp, vp]
+        L.corr_fstage_destroy.restype, L.corr_fstage_destroy.argtypes = ci, [vp]
+        L.corr_fstage_in_bytes.restype, L.corr_fstage_in_bytes.argtypes = ctypes.c_size_t, [vp]
+        L.corr_fstage_out_bytes.restype, L.corr_fstage_out_bytes.argtypes = ctypes.c_size_t, [vp]
         L.corr_stream_run.restype = ci
         L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
         _lib = L
@@ -174,6 +180,48 @@ def probe_mma(m=128, n=256, mn_major=True, iters=4096, random_fill=False):
     if lib().corr_probe_mma(m, n, (1 if mn_major else 0) | (2 if random_fill else 0), iters, out) != CORR_OK:
         _raise()
     return {"ms": out[0], "cycles_per_mma": out[1], "tops": out[2], "sm_mhz": out[3]}
+
+
+class FStage:
+    """The F-stage in front of the float X-engine (corr_fstage_*): raw complex-int8 voltages
+    [n_batch][n_fft][n_inputs][2] -> float32 spectra [n_batch][n_fft][n_inputs][2]."""
+
+    def __init__(self, n_inputs, n_fft, n_batch):
+        self.n_inputs, self.n_fft, self.n_batch = n_inputs, n_fft, n_batch
+        self._f = lib().corr_fstage_create(n_inputs, n_fft, n_batch)
+        if not self._f:
+            _raise()
+        self.in_bytes = lib().corr_fstage_in_bytes(self._f)
+        self.out_bytes = lib().corr_fstage_out_bytes(self._f)
+
+    def run(self, d_raw, d_spec=None, stream=None):
+        import torch
+        if not d_raw.is_cuda or not d_raw.is_contiguous() or d_raw.numel() * d_raw.element_size() != self.in_bytes:
+            raise ValueError(f"d_raw must be a contiguous CUDA tensor of {self.in_bytes} bytes ([B][n_fft][N][2] int8)")
+        if d_spec is None:
+            d_spec = torch.empty((self.n_batch, self.n_fft, self.n_inputs, 2), dtype=torch.float32, device="cuda")
+        if not d_spec.is_cuda or not d_spec.is_contiguous() or d_spec.numel() * d_spec.element_size() != self.out_bytes:
+            raise ValueError(f"d_spec must be a contiguous CUDA tensor of {self.out_bytes} bytes")
+        if lib().corr_fstage_run(self._f, d_raw.data_ptr(), d_spec.data_ptr(), _stream_ptr(stream)) != CORR_OK:
+            _raise()
+        return d_spec
+
+    def destroy(self):
+        if getattr(self, "_f", None) and lib is not None:
+            lib().corr_fstage_destroy(self._f)
+            self._f = None
+
+
+def corr_fstage_create(n_inputs, n_fft, n_batch):
+    return FStage(n_inputs, n_fft, n_batch)
+
+
+def corr_fstage_run(f, d_raw, d_spec=None, stream=None):
+    return f.run(d_raw, d_spec, stream)
+
+
+def corr_fstage_destroy(f):
+    f.destroy()
 
 
 def corr_create(n_inputs, n_chan, n_time, dtype):

@@ -12,10 +12,12 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <cmath>
 #include <queue>
 #include <vector>
 
 #include "corner_turn.cuh"
+#include "fengine.cuh"
 #include "probe_mma.cuh"
 #include "xengine_f32.cuh"
 #include "xengine_i8.cuh"
@@ -566,5 +568,79 @@ int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
   for (cudaEvent_t &e : ev) cudaEventDestroy(e);
   return rc;
 }
+
+// ---------------------------------------------------------------------------- F-stage
+struct corr_fstage {
+  int n_inputs, n_fft, n_batch;
+  size_t in_bytes, out_bytes;
+};
+
+corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
+  g_status = CORR_OK;
+  g_err[0] = 0;
+  if (n_inputs <= 0 || n_fft <= 0 || n_batch <= 0) {
+    fail(CORR_EINVAL, "corr_fstage_create: n_inputs, n_fft, n_batch must be positive (got %d, %d, %d)", n_inputs, n_fft, n_batch);
+    return nullptr;
+  }
+  if (n_fft != corr::kFftN) {
+    fail(CORR_EUNSUPPORTED, "corr_fstage_create: n_fft must be 128 (the paper's N_C, PAPER.md:164; got %d)", n_fft);
+    return nullptr;
+  }
+  if (n_inputs % corr::kFftTile != 0 || n_inputs > 4096) {
+    fail(CORR_EUNSUPPORTED, "corr_fstage_create: n_inputs must be a multiple of 32 and <= 4096 (got %d)", n_inputs);
+    return nullptr;
+  }
+  if (static_cast<long long>(n_batch) * (n_inputs / corr::kFftTile) > 0x7fffffffLL) {
+    fail(CORR_EUNSUPPORTED, "corr_fstage_create: n_batch * n_inputs too large");
+    return nullptr;
+  }
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    fail(CORR_ECUDA, "corr_fstage_create: no usable CUDA device (%s)", cudaGetErrorString(cudaGetLastError()));
+    return nullptr;
+  }
+  if (prop.major != 10) {
+    fail(CORR_EARCH, "corr_fstage_create: device is sm_%d%d, this library is built for sm_100a only", prop.major, prop.minor);
+    return nullptr;
+  }
+  // twiddles exp(-2 pi i m / 128) in float64, rounded once to float32
+  float2 tw[corr::kFftN];
+  for (int m = 0; m < corr::kFftN; ++m) {
+    const double phi = 2.0 * 3.14159265358979323846 * m / corr::kFftN;
+    tw[m] = make_float2(static_cast<float>(cos(phi)), static_cast<float>(-sin(phi)));
+  }
+  if (cudaMemcpyToSymbol(corr::c_tw128, tw, sizeof tw) != cudaSuccess) {
+    fail(CORR_ECUDA, "corr_fstage_create: cudaMemcpyToSymbol: %s", cudaGetErrorString(cudaGetLastError()));
+    return nullptr;
+  }
+  corr_fstage *f = new (std::nothrow) corr_fstage();
+  if (!f) { fail(CORR_EALLOC, "corr_fstage_create: out of host memory"); return nullptr; }
+  f->n_inputs = n_inputs; f->n_fft = n_fft; f->n_batch = n_batch;
+  f->in_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 2;
+  f->out_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 8;
+  return f;
+}
+
+int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *stream) {
+  if (!f || !d_raw || !d_spec) return fail(CORR_EINVAL, "corr_fstage_run: NULL argument");
+  if ((reinterpret_cast<uintptr_t>(d_raw) & 15) || (reinterpret_cast<uintptr_t>(d_spec) & 15))
+    return fail(CORR_EINVAL, "corr_fstage_run: pointers must be 16-byte aligned");
+  corr::FftParams p;
+  p.raw = static_cast<const int8_t *>(d_raw);
+  p.spec = static_cast<float2 *>(d_spec);
+  p.n_batch = f->n_batch; p.n_inputs = f->n_inputs; p.tiles_per_batch = f->n_inputs / corr::kFftTile;
+  corr::fengine_kernel<<<f->n_batch * p.tiles_per_batch, corr::kFftThreads, 0, static_cast<cudaStream_t>(stream)>>>(p);
+  CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
+int corr_fstage_destroy(corr_fstage *f) {
+  delete f;
+  return CORR_OK;
+}
+
+size_t corr_fstage_in_bytes(const corr_fstage *f) { return f ? f->in_bytes : 0; }
+size_t corr_fstage_out_bytes(const corr_fstage *f) { return f ? f->out_bytes : 0; }
 
 }  // extern "C"

@@ -50,6 +50,16 @@ def test_no_cpu_fallback_without_device():
     L = pkg.lib()
     assert L.corr_destroy(None) == pkg.CORR_OK
     assert L.corr_xengine(None, None, None, None) == pkg.CORR_EINVAL
+    # F-stage: same rules (no device -> error code; bad shapes rejected before any device work)
+    with pytest.raises(pkg.CorrError) as e:
+        pkg.corr_fstage_create(64, 128, 10)
+    assert e.value.status in (pkg.CORR_ECUDA, pkg.CORR_EARCH)
+    for bad in [(64, 64, 10), (48, 128, 10), (64, 128, 0)]:
+        with pytest.raises(pkg.CorrError) as e:
+            pkg.corr_fstage_create(*bad)
+        assert e.value.status in (pkg.CORR_EINVAL, pkg.CORR_EUNSUPPORTED)
+    assert L.corr_fstage_destroy(None) == pkg.CORR_OK
+    assert L.corr_fstage_run(None, None, None, None) == pkg.CORR_EINVAL
 
 
 def _imports(path):
