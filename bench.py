@@ -342,6 +342,46 @@ def packed_entry(pkg, torch, peaks, steps=50, warmup=5):
     return out
 
 
+def fstage_entry(pkg, torch, peaks, steps=50, warmup=5):
+    """the F-stage on the raw voltages of one c5 integration (500 spectra x 12 bands of 128
+    channels x 64 inputs, complex int8 -> float32 spectra), then F + X back to back (raw voltages -> visibilities).
+    HBM-bound: algorithmic bytes = 2 B read + 8 B written per sample."""
+    import corrgen
+    w = corrgen.CONFIGS["c5"]
+    bands = w.n_chan // 128
+    B = w.n_time * bands
+    raw = torch.from_numpy(corrgen.gauss_i8(B, 128, w.n_inputs, 4, 4.0, 15.0)).cuda()   # 5-bit Gaussian voltages
+    f = pkg.corr_fstage_create(w.n_inputs, 128, B)
+    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, "cf32")
+    spec = torch.empty((w.n_time, w.n_chan, w.n_inputs, 2), dtype=torch.float32, device="cuda")
+    vis = h.empty_vis()
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ev[0].record(stream)
+        for k in range(steps):
+            fn()
+            ev[k + 1].record(stream)
+        torch.cuda.synchronize()
+        per = sorted(ev[k].elapsed_time(ev[k + 1]) * 1e-3 for k in range(steps))
+        return per[len(per) // 2]
+
+    sec_f = timed(lambda: f.run(raw, spec, stream))
+    sec_fx = timed(lambda: (f.run(raw, spec, stream), h.xengine(spec, vis, stream)))
+    nbytes = f.in_bytes + f.out_bytes
+    t_a = nbytes / (peaks["hbm_gbs"] * 1e9)
+    out = {"n_inputs": w.n_inputs, "dtype": "s8 -> f32 (128-point forward transform)", "batch": B,
+           "ms": sec_f * 1e3, "bytes": nbytes, "achieved_gbs": nbytes / sec_f / 1e9, "bound": "hbm",
+           "roofline_ms": t_a * 1e3, "frac": t_a / sec_f, "samples_per_s": B * 128 * w.n_inputs / sec_f,
+           "fx_ms": sec_fx * 1e3, "fx_value": w.cmacs / sec_fx, "unit": UNIT}
+    f.destroy()
+    h.destroy()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -446,6 +486,10 @@ def main():
             sweep["c2_4bit"] = packed_entry(pkg, torch, peaks)
         except Exception as e:
             sweep["c2_4bit"] = {"error": str(e)[:200]}
+        try:
+            sweep["c5_fstage"] = fstage_entry(pkg, torch, peaks)
+        except Exception as e:
+            sweep["c5_fstage"] = {"error": str(e)[:200]}
         line["by_config"] = sweep
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -590,7 +590,7 @@ corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
     fail(CORR_EUNSUPPORTED, "corr_fstage_create: n_inputs must be a multiple of 32 and <= 4096 (got %d)", n_inputs);
     return nullptr;
   }
-  if (static_cast<long long>(n_batch) * (n_inputs / corr::kFftTile) > 0x7fffffffLL) {
+  if (static_cast<long long>(n_batch) * corr::kFftN * n_inputs > 0x7fffffffLL) {  // 32-bit element offsets
     fail(CORR_EUNSUPPORTED, "corr_fstage_create: n_batch * n_inputs too large");
     return nullptr;
   }

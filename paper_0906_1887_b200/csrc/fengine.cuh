@@ -35,8 +35,20 @@ struct FftParams {
 
 __constant__ float2 c_tw128[kFftN];  // exp(-2 pi i m / 128), filled by corr_fstage_create (float64 -> float32)
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex add / subtract as ONE packed instruction (add.f32x2 / sub.f32x2, sm_100): the transform is mostly
+// complex additions and the FP32 pipes, not HBM, were the limit with scalar FADDs.
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+  float2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(reinterpret_cast<unsigned long long &>(r))
+      : "l"(reinterpret_cast<const unsigned long long &>(a)), "l"(reinterpret_cast<const unsigned long long &>(b)));
+  return r;
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+  float2 r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(reinterpret_cast<unsigned long long &>(r))
+      : "l"(reinterpret_cast<const unsigned long long &>(a)), "l"(reinterpret_cast<const unsigned long long &>(b)));
+  return r;
+}
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
   return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x);
 }
@@ -44,8 +56,10 @@ __device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.
 
 // 4-point forward transform, in place, natural order out
 __device__ __forceinline__ void fft4(float2 &x0, float2 &x1, float2 &x2, float2 &x3) {
-  const float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = mul_mi(csub(x1, x3));
-  x0 = cadd(t0, t2); x1 = cadd(t1, t3); x2 = csub(t0, t2); x3 = csub(t1, t3);
+  const float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), d = csub(x1, x3);
+  x0 = cadd(t0, t2); x2 = csub(t0, t2);
+  x1 = make_float2(t1.x + d.y, t1.y - d.x);  // t1 + (-i) d
+  x3 = make_float2(t1.x - d.y, t1.y + d.x);  // t1 - (-i) d
 }
 
 // 8-point forward transform: v[n] -> v[k], natural order
@@ -93,24 +107,35 @@ __device__ __forceinline__ void fft16(float2 (&v)[16]) {
     }
 }
 
-__global__ void __launch_bounds__(kFftThreads)
+__global__ void __launch_bounds__(kFftThreads, 4)
 fengine_kernel(const FftParams p) {
   __shared__ float2 z[kFftN * kFftTile];  // [n2][k1][lane], 32 KB
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;  // pass 1: n2; pass 2: k1 (and k1 + 8)
-  const int b = blockIdx.x / p.tiles_per_batch;
-  const int i = (blockIdx.x - b * p.tiles_per_batch) * kFftTile + lane;
-  const size_t base = static_cast<size_t>(b) * kFftN * p.n_inputs + i;
+  // CTA = (batch, input tile), tile fastest: the tiles of one batch run side by side, so that the 256-byte
+  // row pieces they write meet in L2 / the same DRAM pages.  Element offsets fit 32 bits (corr_fstage_create).
+  const uint32_t ni = static_cast<uint32_t>(p.n_inputs);
+  const uint32_t b = blockIdx.x / static_cast<uint32_t>(p.tiles_per_batch);
+  const uint32_t tile = blockIdx.x - b * static_cast<uint32_t>(p.tiles_per_batch);
+  const uint32_t base = b * (kFftN * ni) + tile * kFftTile + lane;
 
   // ---- pass 1: unpack (int8 -> float) + 16-point transforms over n1 for residue n2 = w
   {
-    const char2 *src = reinterpret_cast<const char2 *>(p.raw) + base + static_cast<size_t>(w) * p.n_inputs;
+    const char2 *src = reinterpret_cast<const char2 *>(p.raw) + (base + w * ni);
     char2 raw[16];
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) raw[n1] = src[static_cast<size_t>(8 * n1) * p.n_inputs];  // all 16 loads in flight
+    for (int n1 = 0; n1 < 16; ++n1) raw[n1] = src[8u * n1 * ni];  // all 16 loads in flight
+    // unpack ("converting to floating-point format") without the quarter-rate I2F: the byte u = x ^ 0x80
+    // placed in the mantissa of 2^23 is the float 8388608 + u; subtracting 8388736 leaves x exactly
     float2 v[16];
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) v[n1] = make_float2(static_cast<float>(raw[n1].x), static_cast<float>(raw[n1].y));
+    for (int n1 = 0; n1 < 16; ++n1) {
+      const uint32_t u = (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].x)) |
+                          (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].y)) << 8)) ^ 0x8080u;
+      const float2 m = make_float2(__uint_as_float(__byte_perm(u, 0x4B000000u, 0x7440)),
+                                   __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441)));
+      v[n1] = csub(m, make_float2(8388736.0f, 8388736.0f));
+    }
     fft16(v);
 #pragma unroll
     for (int k1 = 0; k1 < 16; ++k1) {
@@ -127,9 +152,9 @@ fengine_kernel(const FftParams p) {
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) v[n2] = z[(n2 * 16 + k1) * kFftTile + lane];
     fft8(v);
-    float2 *dst = p.spec + base + static_cast<size_t>(k1) * p.n_inputs;
+    float2 *dst = p.spec + (base + k1 * ni);
 #pragma unroll
-    for (int k2 = 0; k2 < 8; ++k2) dst[static_cast<size_t>(16 * k2) * p.n_inputs] = v[k2];
+    for (int k2 = 0; k2 < 8; ++k2) dst[16u * k2 * ni] = v[k2];
   }
 }
 
