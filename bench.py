@@ -377,6 +377,18 @@ def fstage_entry(pkg, torch, peaks, steps=50, warmup=5):
            "ms": sec_f * 1e3, "bytes": nbytes, "achieved_gbs": nbytes / sec_f / 1e9, "bound": "hbm",
            "roofline_ms": t_a * 1e3, "frac": t_a / sec_f, "samples_per_s": B * 128 * w.n_inputs / sec_f,
            "fx_ms": sec_fx * 1e3, "fx_value": w.cmacs / sec_fx, "unit": UNIT}
+    # the streaming driver fed with raw voltages (corr_stream_run_fx): a quarter of the PCIe bytes per integration
+    ring = [torch.from_numpy(corrgen.gauss_i8(B, 128, w.n_inputs, 40 + k, 4.0, 15.0)).pin_memory() for k in range(4)]
+    hs = [ring[k % 4] for k in range(w.n_integrations)]
+    h.stream_run(hs, fstage=f)  # warm-up (allocates the device buffers)
+    _, st = h.stream_run(hs, fstage=f)
+    rate = w.n_integrations * w.n_time * w.n_chan / st["device_s"]
+    out["stream_fx"] = {"integrations": w.n_integrations, "device_s": st["device_s"], "kernel_s": st["kernel_s"],
+                        "h2d_s": st["h2d_s"], "h2d_bytes_per_integration": f.in_bytes,
+                        "h2d_gbs": w.n_integrations * f.in_bytes / st["h2d_s"] / 1e9,
+                        "samples_per_s_per_input": rate, "rtf_vs_15.36MSps": rate / 15.36e6,
+                        "rtf_vs_paper_1.28MSps": rate / 1.28e6,
+                        "e2e_cmacs_per_s": w.n_integrations * w.cmacs / st["device_s"]}
     f.destroy()
     h.destroy()
     return out

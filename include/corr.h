@@ -174,7 +174,7 @@ int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
  * <= 4096, n_batch >= 1; NULL + corr_last_error() otherwise (CORR_EINVAL / CORR_EUNSUPPORTED / CORR_EARCH /
  * CORR_ECUDA / CORR_EALLOC).  corr_fstage_run is asynchronous on `stream`; returns CORR_OK, CORR_EINVAL or
  * CORR_ECUDA.  FP32 arithmetic: |dX| <= 1e-5 * ||x[b][:][i]||_2 per channel against the float64 definition
- * (DESIGN.md section 6).  The handle owns nothing on the device; corr_fstage_destroy(NULL) is a no-op.
+ * (DESIGN.md section 6).  The handle owns device memory only once corr_stream_run_fx has been used; corr_fstage_destroy(NULL) is a no-op.
  */
 typedef struct corr_fstage corr_fstage; /* opaque */
 corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch);
@@ -182,6 +182,19 @@ int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *strea
 int corr_fstage_destroy(corr_fstage *f);
 size_t corr_fstage_in_bytes(const corr_fstage *f);  /* n_batch * n_fft * n_inputs * 2 */
 size_t corr_fstage_out_bytes(const corr_fstage *f); /* n_batch * n_fft * n_inputs * 8 */
+
+/*
+ * corr_stream_run_fx -- the streaming driver fed with RAW VOLTAGES: per integration the
+ * host->device copy moves corr_fstage_in_bytes(f) bytes of complex int8 (a quarter of the float spectra),
+ * then F-stage and X-engine run back to back on the compute stream while the next copy is in flight --
+ * the paper's whole chain unpack -> FFT -> CMAC on the device.
+ *   h     : CORR_CF32 handle with n_time * n_chan * n_inputs == n_batch * n_fft * n_inputs of f
+ *   h_raw : n_integrations pointers to PINNED host buffers of corr_fstage_in_bytes(f) bytes
+ *   d_vis, stats : as corr_stream_run ([2] = sum of F + X kernel seconds).
+ * The F-stage handle owns two raw buffers and one spectra buffer on the device from the first call on.
+ */
+int corr_stream_run_fx(corr_handle *h, corr_fstage *f, const void *const *h_raw, int n_integrations,
+                       void *d_vis, double *stats);
 
 #ifdef __cplusplus
 }

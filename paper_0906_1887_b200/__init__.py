@@ -19,7 +19,7 @@ CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
            "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize",
-           "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes")
+           "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx")
 
 _lib = None
 
@@ -60,6 +60,8 @@ def lib():
         L.corr_fstage_destroy.restype, L.corr_fstage_destroy.argtypes = ci, [vp]
         L.corr_fstage_in_bytes.restype, L.corr_fstage_in_bytes.argtypes = ctypes.c_size_t, [vp]
         L.corr_fstage_out_bytes.restype, L.corr_fstage_out_bytes.argtypes = ctypes.c_size_t, [vp]
+        L.corr_stream_run_fx.restype = ci
+        L.corr_stream_run_fx.argtypes = [vp, vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
         L.corr_stream_run.restype = ci
         L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
         _lib = L
@@ -158,17 +160,22 @@ class Correlator:
         return d_out
 
     # -- corr_stream_run
-    def stream_run(self, h_in_list, d_vis=None):
-        """h_in_list: pinned host tensors, one per integration.  Returns (d_vis, stats dict)."""
+    def stream_run(self, h_in_list, d_vis=None, fstage=None):
+        """h_in_list: pinned host tensors, one per integration (raw int8 voltages when `fstage` is given:
+        corr_stream_run_fx).  Returns (d_vis, stats dict)."""
         n = len(h_in_list)
+        want = self.in_bytes if fstage is None else fstage.in_bytes
         for t in h_in_list:
-            if t.is_cuda or not t.is_pinned() or t.numel() * t.element_size() != self.in_bytes:
-                raise ValueError("stream_run needs pinned host tensors of in_bytes each")
+            if t.is_cuda or not t.is_pinned() or t.numel() * t.element_size() != want:
+                raise ValueError(f"stream_run needs pinned host tensors of {want} bytes each")
         if d_vis is None:
             d_vis = self.empty_vis(n)
         ptrs = (ctypes.c_void_p * n)(*[t.data_ptr() for t in h_in_list])
         stats = (ctypes.c_double * 4)()
-        rc = lib().corr_stream_run(self._h, ptrs, n, d_vis.data_ptr(), stats)
+        if fstage is None:
+            rc = lib().corr_stream_run(self._h, ptrs, n, d_vis.data_ptr(), stats)
+        else:
+            rc = lib().corr_stream_run_fx(self._h, fstage._f, ptrs, n, d_vis.data_ptr(), stats)
         if rc != CORR_OK:
             _raise()
         return d_vis, {"wall_s": stats[0], "device_s": stats[1], "kernel_s": stats[2], "h2d_s": stats[3]}

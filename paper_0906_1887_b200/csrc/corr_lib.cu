@@ -87,6 +87,13 @@ struct corr_handle {
   cudaStream_t s_copy, s_compute;
 };
 
+struct corr_fstage {
+  int n_inputs, n_fft, n_batch;
+  size_t in_bytes, out_bytes;
+  void *d_raw[2];  // streaming driver: double-buffered raw voltages
+  void *d_spec;    // streaming driver: spectra of the integration in flight
+};
+
 namespace {
 
 // Schedule planning (host side of the uniform decode in xengine_i8.cuh).
@@ -517,17 +524,39 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   return CORR_OK;
 }
 
+static int stream_run_impl(corr_handle *h, corr_fstage *f, const void *const *h_in, int n_integrations, void *d_vis,
+                           double *stats);
+
 int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations, void *d_vis, double *stats) {
+  return stream_run_impl(h, nullptr, h_in, n_integrations, d_vis, stats);
+}
+
+int corr_stream_run_fx(corr_handle *h, corr_fstage *f, const void *const *h_raw, int n_integrations, void *d_vis,
+                       double *stats) {
+  if (!f) return fail(CORR_EINVAL, "corr_stream_run_fx: NULL F-stage handle");
+  if (!h || h->dtype != CORR_CF32 || h->in_bytes != f->out_bytes || h->n_inputs != f->n_inputs)
+    return fail(CORR_EINVAL, "corr_stream_run_fx: the X-engine handle must be CORR_CF32 with n_time * n_chan = n_batch * n_fft");
+  return stream_run_impl(h, f, h_raw, n_integrations, d_vis, stats);
+}
+
+static int stream_run_impl(corr_handle *h, corr_fstage *f, const void *const *h_in, int n_integrations, void *d_vis,
+                           double *stats) {
   if (!h || !h_in || !d_vis || n_integrations <= 0) return fail(CORR_EINVAL, "corr_stream_run: bad argument");
   for (int k = 0; k < n_integrations; ++k)
     if (!h_in[k]) return fail(CORR_EINVAL, "corr_stream_run: h_in[%d] is NULL", k);
   if (!h->s_copy) CUDA_TRY(cudaStreamCreateWithFlags(&h->s_copy, cudaStreamNonBlocking));
   if (!h->s_compute) CUDA_TRY(cudaStreamCreateWithFlags(&h->s_compute, cudaStreamNonBlocking));
+  const size_t copy_bytes = f ? f->in_bytes : h->in_bytes;
+  void **d_buf = f ? f->d_raw : h->d_stream_in;
   for (int b = 0; b < 2; ++b)
-    if (!h->d_stream_in[b]) {
-      cudaError_t e = cudaMalloc(&h->d_stream_in[b], h->in_bytes);
-      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_stream_run: input buffer of %zu bytes: %s", h->in_bytes, cudaGetErrorString(e));
+    if (!d_buf[b]) {
+      cudaError_t e = cudaMalloc(&d_buf[b], copy_bytes);
+      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_stream_run: input buffer of %zu bytes: %s", copy_bytes, cudaGetErrorString(e));
     }
+  if (f && !f->d_spec) {
+    cudaError_t e = cudaMalloc(&f->d_spec, f->out_bytes);
+    if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_stream_run_fx: spectra buffer of %zu bytes: %s", f->out_bytes, cudaGetErrorString(e));
+  }
   const int n = n_integrations;
   std::vector<cudaEvent_t> ev(4 * n);  // per integration: copy start, copy end, kernel start, kernel end
   for (cudaEvent_t &e : ev) CUDA_TRY(cudaEventCreate(&e));
@@ -538,11 +567,17 @@ int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
     // buffer b is free once the kernel of integration k-2 has finished reading it
     if (k >= 2) cudaStreamWaitEvent(h->s_copy, ev[4 * (k - 2) + 3], 0);
     cudaEventRecord(ev[4 * k + 0], h->s_copy);
-    cudaMemcpyAsync(h->d_stream_in[b], h_in[k], h->in_bytes, cudaMemcpyHostToDevice, h->s_copy);
+    cudaMemcpyAsync(d_buf[b], h_in[k], copy_bytes, cudaMemcpyHostToDevice, h->s_copy);
     cudaEventRecord(ev[4 * k + 1], h->s_copy);
     cudaStreamWaitEvent(h->s_compute, ev[4 * k + 1], 0);
     cudaEventRecord(ev[4 * k + 2], h->s_compute);
-    rc = corr_xengine(h, h->d_stream_in[b], static_cast<char *>(d_vis) + static_cast<size_t>(k) * h->vis_bytes, h->s_compute);
+    const void *x_in = d_buf[b];
+    if (f) {  // raw voltages -> spectra (one buffer: F and X of integration k are ordered on the compute stream)
+      rc = corr_fstage_run(f, d_buf[b], f->d_spec, h->s_compute);
+      x_in = f->d_spec;
+    }
+    if (rc == CORR_OK)
+      rc = corr_xengine(h, x_in, static_cast<char *>(d_vis) + static_cast<size_t>(k) * h->vis_bytes, h->s_compute);
     cudaEventRecord(ev[4 * k + 3], h->s_compute);
   }
   cudaError_t e1 = cudaStreamSynchronize(h->s_copy);
@@ -570,10 +605,6 @@ int corr_stream_run(corr_handle *h, const void *const *h_in, int n_integrations,
 }
 
 // ---------------------------------------------------------------------------- F-stage
-struct corr_fstage {
-  int n_inputs, n_fft, n_batch;
-  size_t in_bytes, out_bytes;
-};
 
 corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
   g_status = CORR_OK;
@@ -617,6 +648,7 @@ corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
   corr_fstage *f = new (std::nothrow) corr_fstage();
   if (!f) { fail(CORR_EALLOC, "corr_fstage_create: out of host memory"); return nullptr; }
   f->n_inputs = n_inputs; f->n_fft = n_fft; f->n_batch = n_batch;
+  f->d_raw[0] = f->d_raw[1] = f->d_spec = nullptr;
   f->in_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 2;
   f->out_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 8;
   return f;
@@ -636,6 +668,11 @@ int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *strea
 }
 
 int corr_fstage_destroy(corr_fstage *f) {
+  if (f) {
+    cudaFree(f->d_raw[0]);
+    cudaFree(f->d_raw[1]);
+    cudaFree(f->d_spec);
+  }
   delete f;
   return CORR_OK;
 }

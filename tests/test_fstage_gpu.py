@@ -108,3 +108,26 @@ def test_fstage_full_size_sampled(pkg):
     e_t = 128.0 * (x.astype(np.float64) ** 2).sum(axis=(1, 3))
     assert np.allclose(e_f, e_t, rtol=2e-6)
     pkg.corr_fstage_destroy(f)
+
+
+def test_stream_run_fx_matches_float64_chain(pkg):
+    """corr_stream_run_fx: pinned raw voltages -> H2D (double-buffered) -> F -> X, three integrations."""
+    T, bands, I, n_int = 10, 1, 32, 3
+    raws = [raw_voltages(T * bands, I, seed=20 + k, tone=3 + k) for k in range(n_int)]
+    f = pkg.corr_fstage_create(I, 128, T * bands)
+    h = pkg.corr_create(I, bands * 128, T, "cf32")
+    pinned = [torch.from_numpy(r).pin_memory() for r in raws]
+    d_vis, stats = h.stream_run(pinned, fstage=f)
+    torch.cuda.synchronize()
+    assert stats["device_s"] > 0 and stats["kernel_s"] > 0
+    out = d_vis.cpu().numpy()
+    for k in range(n_int):
+        ref_spec = oracle.fstage_ci8(raws[k], threads=oracle.host_threads()).reshape(T, bands * 128, I, 2)
+        f32_tolerance_check(out[k], oracle.xengine_cf64(ref_spec, threads=oracle.host_threads()), I, rel=2e-5)
+    # a handle of another shape is refused
+    h2 = pkg.corr_create(I, 128, T + 1, "cf32")
+    with pytest.raises(pkg.CorrError):
+        h2.stream_run([torch.from_numpy(raws[0]).pin_memory()], fstage=f)
+    pkg.corr_destroy(h2)
+    pkg.corr_destroy(h)
+    pkg.corr_fstage_destroy(f)
