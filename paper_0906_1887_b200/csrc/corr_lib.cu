@@ -198,6 +198,10 @@ void plan_i8(corr_handle *h) {
   ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ring_bytes);
   h->smem_i8 = static_cast<size_t>(ring_bytes) * ip.stages + epi_bytes + bar_bytes;
   ip.units = std::min(ip.n_items, ip.pair2 ? h->n_sms / 2 : h->n_sms);
+  if (const char *ue = getenv("CORR_UNITS")) {  // experiments: fewer, fatter CTAs
+    const int u = atoi(ue);
+    if (u >= 1 && !ip.pair2) ip.units = std::min(ip.units, u);
+  }
   h->grid_i8 = ip.pair2 ? 2 * ip.units : ip.units;
   const int deltas[2] = {ip.units + ip.rot, ip.rot};
   for (int w = 0; w < 2; ++w) { ip.dq[w] = deltas[w] / ip.n_kinds; ip.dr[w] = deltas[w] % ip.n_kinds; }
