@@ -161,10 +161,10 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
     it.xa = xc + it.I * kPanelBytes; it.za = it.z0;
   }
   if (!p.pair2) { it.nblk_load = it.nblk; it.jperm = 0; }
-  if (it.n_load == 1)      { it.bk = 256; it.map = 0; }
-  else if (it.n_load == 2) { it.bk = 128; it.map = 1; }
-  else if (it.n_load == 3 && p.stage_bytes >= 3 * 128 * kPanelBytes) { it.bk = 128; it.map = 1; }
-  else                     { it.bk = 64;  it.map = 2; }
+  // the tallest box (256 / 128 / 64 time rows) whose n_load panels fit one stage
+  if (it.n_load * 256 * kPanelBytes <= p.stage_bytes)      { it.bk = 256; it.map = 0; }
+  else if (it.n_load * 128 * kPanelBytes <= p.stage_bytes) { it.bk = 128; it.map = 1; }
+  else                                                     { it.bk = 64;  it.map = 2; }
   return it;
 }
 
