@@ -20,6 +20,7 @@
 #include "fengine.cuh"
 #include "probe_mma.cuh"
 #include "xengine_f32.cuh"
+#include "xengine_f32_n64.cuh"
 #include "xengine_i8.cuh"
 
 namespace {
@@ -82,6 +83,7 @@ struct corr_handle {
   int2 *d_items_f32;
   int n_items_f32;
   int f32_threads;
+  int n64_groups, n64_slices, n64_slice_len;  // CF32 with N_I = 64: xengine_f32_n64_kernel
   // streaming driver
   void *d_stream_in[2];
   cudaStream_t s_copy, s_compute;
@@ -213,6 +215,21 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
     for (int I = 0; I < blocks; ++I)
       for (int J = 0; J <= I; ++J) items.push_back(make_int2(c, I | (J << 16)));
   h->n_items_f32 = static_cast<int>(items.size());
+  // N_I = 64: (8-channel group, time slice) units; as many slices as fill the SMs evenly (cost = rounds x rows per
+  // slice, plus 32 rows for the zeroing node and the reduce-adds of a sliced plan)
+  h->n64_groups = h->n64_slices = h->n64_slice_len = 0;
+  if (h->n_inputs == 64 && !getenv("CORR_F32_GENERIC")) {
+    const int T = h->n_time, G = h->n_sms;
+    h->n64_groups = (h->n_chan + corr::kN64Chan - 1) / corr::kN64Chan;
+    long long best = -1;
+    for (int sl = 1; sl <= 32; ++sl) {
+      const int len = ((T + sl - 1) / sl + corr::kN64TB - 1) / corr::kN64TB * corr::kN64TB;
+      if ((T + len - 1) / len != sl) continue;
+      const long long rounds = (1LL * h->n64_groups * sl + G - 1) / G;
+      const long long cost = rounds * len + (sl > 1 ? 32 : 0);
+      if (best < 0 || cost < best) { best = cost; h->n64_slices = sl; h->n64_slice_len = len; }
+    }
+  }
   h->f32_threads = blocks == 1 ? 160 : corr::kF32Threads;  // 136 active tiles on a diagonal block
 }
 
@@ -337,6 +354,8 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
     plan_f32(h, items);
     e = cudaMalloc(&h->d_items_f32, items.size() * sizeof(int2));
     if (e == cudaSuccess) e = cudaMemcpy(h->d_items_f32, items.data(), items.size() * sizeof(int2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && h->n64_groups > 0)
+      e = cudaFuncSetAttribute(corr::xengine_f32_n64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::kN64Smem);
   }
   if (e != cudaSuccess) {
     fail(e == cudaErrorMemoryAllocation ? CORR_EALLOC : CORR_ECUDA, "corr_create: %s", cudaGetErrorString(e));
@@ -490,6 +509,18 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   if (d_in == d_vis) return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis alias");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (h->dtype == CORR_CF32) {
+    if (h->n64_groups > 0) {
+      corr::F32N64Params np;
+      np.in = static_cast<const float2 *>(d_in);
+      np.vis = static_cast<float2 *>(d_vis);
+      np.n_time = h->n_time; np.n_chan = h->n_chan;
+      np.n_groups = h->n64_groups; np.n_slices = h->n64_slices; np.slice_len = h->n64_slice_len;
+      np.add = (h->n64_slices > 1 || h->accumulate) ? 1 : 0;
+      if (h->n64_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));
+      corr::xengine_f32_n64_kernel<<<h->n64_groups * h->n64_slices, corr::kN64Threads, corr::kN64Smem, st>>>(np);
+      CUDA_TRY(cudaGetLastError());
+      return CORR_OK;
+    }
     corr::F32Params fp;
     fp.in = static_cast<const float2 *>(d_in);
     fp.vis = static_cast<float2 *>(d_vis);
