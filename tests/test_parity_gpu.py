@@ -224,3 +224,15 @@ def test_ci8_diag_plans_bit_exact(pkg, monkeypatch, plan, N, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
     assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+
+
+# N_I = 64 float path (xengine_f32_n64_kernel: 7-channel groups, time slices with reduce-add): group tails (C not a
+# multiple of 7), slice tails, one slice (plain stores) and many; and the generic 4 x 4 kernel forced on the same shapes.
+@pytest.mark.parametrize("generic", [False, True])
+@pytest.mark.parametrize("C,T", [(1, 1), (7, 16), (8, 17), (15, 100), (150, 33), (23, 700), (300, 260)])
+def test_cf32_n64_paths_within_tolerance(pkg, monkeypatch, generic, C, T):
+    if generic:
+        monkeypatch.setenv("CORR_F32_GENERIC", "1")
+    w = corrgen.scaled(corrgen.CONFIGS["c5"], n_inputs=64, n_chan=C, n_time=T)
+    x = w.generate()
+    f32_tolerance_check(run_cf32(pkg, x), oracle.xengine_cf32(x, threads=_threads()), 64)
