@@ -58,6 +58,7 @@ def _load():
         _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
         _lib.oracle_one_visibility_cf32.argtypes = [P, L, L, L, L, L, L, P]
         _lib.oracle_fstage_ci8.argtypes = [P, L, L, L, P, I]
+        _lib.oracle_fstage_ci4.argtypes = [P, L, L, L, P, I]
         _lib.oracle_xengine_cf64.argtypes = [P, L, L, L, P, I]
     return _lib
 
@@ -171,6 +172,18 @@ def fstage_ci8(x, threads=1):
     B, N, I, _ = x.shape
     out = np.empty((B, N, I, 2), dtype=np.float64)
     rc = _load().oracle_fstage_ci8(x.ctypes.data, B, N, I, out.ctypes.data, int(threads))
+    assert rc == 0
+    return out
+
+
+def fstage_ci4(x, threads=1):
+    """x: [B][N_C][N_I] uint8 (low nibble Re, high nibble Im, 4-bit two's complement: the paper's 1-byte mode,
+    PAPER.md:164) -> [B][N_C][N_I][2] float64 spectra."""
+    x = np.ascontiguousarray(x)
+    assert x.dtype == np.uint8 and x.ndim == 3, (x.dtype, x.shape)
+    B, N, I = x.shape
+    out = np.empty((B, N, I, 2), dtype=np.float64)
+    rc = _load().oracle_fstage_ci4(x.ctypes.data, B, N, I, out.ctypes.data, int(threads))
     assert rc == 0
     return out
 

@@ -62,6 +62,43 @@ int oracle_fstage_ci8(const int8_t *x, long n_batch, long n_fft, long n_inputs, 
 }
 
 /*
+ * The same transform for the paper's "1-byte mode" ("the data samples were reduced from 2-byte words
+ * to a single byte, at the cost of 1 bit of precision in the real and imaginary parts ... reduces the total amount of
+ * global memory reads in the unpack phase"): x is [B][N][I] BYTES, low nibble = Re, high nibble = Im, 4-bit two's
+ * complement (DESIGN reading R18, the same byte as the X-engine's CORR_CI4 input).  The nibble decode is written out
+ * here again (v >= 8 ? v - 16 : v) so that this file stands alone; pin F8 checks it against the int8 routine above on
+ * data unpacked by numpy, and P11's hand-written byte table pins the byte layout.
+ */
+int oracle_fstage_ci4(const uint8_t *x, long n_batch, long n_fft, long n_inputs, double *out, int threads)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    (void)threads;
+#pragma omp parallel for num_threads(threads) schedule(static) if (threads > 1)
+    for (long b = 0; b < n_batch; ++b) {
+        const uint8_t *xb = x + b * n_fft * n_inputs;
+        double *ob = out + 2 * b * n_fft * n_inputs;
+        for (long i = 0; i < n_inputs; ++i) {
+            for (long k = 0; k < n_fft; ++k) {
+                double re = 0.0, im = 0.0;
+                for (long n = 0; n < n_fft; ++n) {
+                    const unsigned byte = xb[n * n_inputs + i];
+                    const unsigned lo = byte & 15u, hi = byte >> 4;
+                    const double a = (double)(lo >= 8 ? (int)lo - 16 : (int)lo); /* Re x[n] */
+                    const double c = (double)(hi >= 8 ? (int)hi - 16 : (int)hi); /* Im x[n] */
+                    const double phi = two_pi * (double)((k * n) % n_fft) / (double)n_fft;
+                    const double wr = cos(phi), wi = -sin(phi);                  /* exp(-i phi) */
+                    re += a * wr - c * wi;
+                    im += a * wi + c * wr;
+                }
+                ob[2 * (k * n_inputs + i)] = re;
+                ob[2 * (k * n_inputs + i) + 1] = im;
+            }
+        }
+    }
+    return 0;
+}
+
+/*
  * The X-engine definition on float64 spectra (same formula and loop order as oracle_xengine_cf32 in
  * xcorr_oracle.c), so that the F -> X chain can be followed in float64 end to end.
  * x : [T][C][N] float64 pairs; vis : [C][N(N+1)/2] float64 pairs.

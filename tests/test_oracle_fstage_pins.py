@@ -114,3 +114,22 @@ def test_f7_float64_xengine_restatement():
     # same numbers as the cf32 oracle when the input is representable in float32
     x32 = x.astype(np.float32)
     assert np.array_equal(oracle.xengine_cf64(x32.astype(np.float64)), oracle.xengine_cf32(x32))
+
+
+def test_f8_one_byte_mode_matches_int8_routine_and_byte_table():
+    """The packed (4+4-bit) F-stage oracle against (a) the int8 routine on data unpacked by numpy with the hand-written
+    table of tests/golden/p11_ci4_unpack.txt semantics (low nibble Re, high nibble Im, two's complement) and (b) numpy.fft."""
+    rng = np.random.default_rng(3)
+    xb = rng.integers(0, 256, size=(3, 16, 5), dtype=np.uint8)          # every byte value can occur
+    lo, hi = (xb & 15).astype(np.int16), (xb >> 4).astype(np.int16)
+    re = np.where(lo >= 8, lo - 16, lo).astype(np.int8)
+    im = np.where(hi >= 8, hi - 16, hi).astype(np.int8)
+    x8 = np.stack([re, im], axis=-1)
+    got = oracle.fstage_ci4(xb, threads=2)
+    assert np.array_equal(got, oracle.fstage_ci8(x8))
+    assert np.max(np.abs(_c(got) - np.fft.fft(_c(x8).astype(np.complex128), axis=1))) < 1e-11
+    # single bytes: 0x7F = 7 - 1i... written out: low nibble F = -1 (Re), high nibble 7 = +7 (Im)
+    one = np.zeros((1, 4, 1), np.uint8)
+    one[0, 0, 0] = 0x7F
+    X = _c(oracle.fstage_ci4(one))[0, :, 0]
+    assert np.allclose(X, (-1 + 7j) * np.ones(4))
