@@ -423,6 +423,17 @@ def fstage_entry(pkg, torch, peaks, steps=50, warmup=5):
                         "samples_per_s_per_input": rate, "rtf_vs_15.36MSps": rate / 15.36e6,
                         "rtf_vs_paper_1.28MSps": rate / 1.28e6,
                         "e2e_cmacs_per_s": w.n_integrations * w.cmacs / st["device_s"]}
+    # the same in the paper's 1-byte mode (4+4-bit raw samples): half the PCIe bytes again
+    raw4 = [torch.from_numpy(corrgen.pack_ci4(corrgen.gauss_i8(B, 128, w.n_inputs, 60 + k, 2.5, 7.0))).pin_memory() for k in range(4)]
+    f.set_input("ci4")
+    hs4 = [raw4[k % 4] for k in range(w.n_integrations)]
+    h.stream_run(hs4, fstage=f)
+    _, st = h.stream_run(hs4, fstage=f)
+    rate = w.n_integrations * w.n_time * w.n_chan / st["device_s"]
+    out["stream_fx_4bit"] = {"integrations": w.n_integrations, "device_s": st["device_s"], "kernel_s": st["kernel_s"],
+                             "h2d_bytes_per_integration": f.in_bytes, "h2d_gbs": w.n_integrations * f.in_bytes / st["h2d_s"] / 1e9,
+                             "samples_per_s_per_input": rate, "rtf_vs_15.36MSps": rate / 15.36e6,
+                             "e2e_cmacs_per_s": w.n_integrations * w.cmacs / st["device_s"]}
     f.destroy()
     h.destroy()
     return out

@@ -180,7 +180,14 @@ typedef struct corr_fstage corr_fstage; /* opaque */
 corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch);
 int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *stream);
 int corr_fstage_destroy(corr_fstage *f);
-size_t corr_fstage_in_bytes(const corr_fstage *f);  /* n_batch * n_fft * n_inputs * 2 */
+/*
+ * corr_fstage_set_input -- raw sample format: CORR_CI8 (default, above) or CORR_CI4, the paper's "1-byte mode"
+ * ("reduced from 2-byte words to a single byte, at the cost of 1 bit of precision ... reduces the
+ * total amount of global memory reads in the unpack phase"): d_raw is [n_batch][n_fft][n_inputs] BYTES, low nibble
+ * Re, high nibble Im, 4-bit two's complement (DESIGN reading R18).  corr_fstage_in_bytes follows.  CORR_EINVAL otherwise.
+ */
+int corr_fstage_set_input(corr_fstage *f, int dtype);
+size_t corr_fstage_in_bytes(const corr_fstage *f);  /* n_batch * n_fft * n_inputs * 2 (CI8) or * 1 (CI4) */
 size_t corr_fstage_out_bytes(const corr_fstage *f); /* n_batch * n_fft * n_inputs * 8 */
 
 /*

@@ -19,7 +19,7 @@ CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
            "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize",
-           "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx")
+           "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx", "corr_fstage_set_input")
 
 _lib = None
 
@@ -58,6 +58,7 @@ def lib():
         L.corr_fstage_create.restype, L.corr_fstage_create.argtypes = vp, [ci, ci, ci]
         L.corr_fstage_run.restype, L.corr_fstage_run.argtypes = ci, [vp, vp, vp, vp]
         L.corr_fstage_destroy.restype, L.corr_fstage_destroy.argtypes = ci, [vp]
+        L.corr_fstage_set_input.restype, L.corr_fstage_set_input.argtypes = ci, [vp, ci]
         L.corr_fstage_in_bytes.restype, L.corr_fstage_in_bytes.argtypes = ctypes.c_size_t, [vp]
         L.corr_fstage_out_bytes.restype, L.corr_fstage_out_bytes.argtypes = ctypes.c_size_t, [vp]
         L.corr_stream_run_fx.restype = ci
@@ -201,10 +202,17 @@ class FStage:
         self.in_bytes = lib().corr_fstage_in_bytes(self._f)
         self.out_bytes = lib().corr_fstage_out_bytes(self._f)
 
+    def set_input(self, dtype):
+        """"ci8" (int8 pairs, default) or "ci4" (one byte per sample, the paper's 1-byte mode)."""
+        code = {"ci8": CORR_CI8, "ci4": CORR_CI4}.get(dtype, dtype)
+        if lib().corr_fstage_set_input(self._f, code) != CORR_OK:
+            _raise()
+        self.in_bytes = lib().corr_fstage_in_bytes(self._f)
+
     def run(self, d_raw, d_spec=None, stream=None):
         import torch
         if not d_raw.is_cuda or not d_raw.is_contiguous() or d_raw.numel() * d_raw.element_size() != self.in_bytes:
-            raise ValueError(f"d_raw must be a contiguous CUDA tensor of {self.in_bytes} bytes ([B][n_fft][N][2] int8)")
+            raise ValueError(f"d_raw must be a contiguous CUDA tensor of {self.in_bytes} bytes ([B][n_fft][N][2] int8, or [B][n_fft][N] bytes in the 4+4-bit mode)")
         if d_spec is None:
             d_spec = torch.empty((self.n_batch, self.n_fft, self.n_inputs, 2), dtype=torch.float32, device="cuda")
         if not d_spec.is_cuda or not d_spec.is_contiguous() or d_spec.numel() * d_spec.element_size() != self.out_bytes:

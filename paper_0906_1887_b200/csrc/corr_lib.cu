@@ -90,7 +90,7 @@ struct corr_handle {
 };
 
 struct corr_fstage {
-  int n_inputs, n_fft, n_batch;
+  int n_inputs, n_fft, n_batch, in_dtype;
   size_t in_bytes, out_bytes;
   void *d_raw[2];  // streaming driver: double-buffered raw voltages
   void *d_spec;    // streaming driver: spectra of the integration in flight
@@ -682,7 +682,7 @@ corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
   }
   corr_fstage *f = new (std::nothrow) corr_fstage();
   if (!f) { fail(CORR_EALLOC, "corr_fstage_create: out of host memory"); return nullptr; }
-  f->n_inputs = n_inputs; f->n_fft = n_fft; f->n_batch = n_batch;
+  f->n_inputs = n_inputs; f->n_fft = n_fft; f->n_batch = n_batch; f->in_dtype = CORR_CI8;
   f->d_raw[0] = f->d_raw[1] = f->d_spec = nullptr;
   f->in_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 2;
   f->out_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 8;
@@ -697,8 +697,24 @@ int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *strea
   p.raw = static_cast<const int8_t *>(d_raw);
   p.spec = static_cast<float2 *>(d_spec);
   p.n_batch = f->n_batch; p.n_inputs = f->n_inputs; p.tiles_per_batch = f->n_inputs / corr::kFftTile;
-  corr::fengine_kernel<<<f->n_batch * p.tiles_per_batch, corr::kFftThreads, 0, static_cast<cudaStream_t>(stream)>>>(p);
+  if (f->in_dtype == CORR_CI4)
+    corr::fengine_ci4_kernel<<<f->n_batch * p.tiles_per_batch, corr::kFftThreads, 0, static_cast<cudaStream_t>(stream)>>>(p);
+  else
+    corr::fengine_kernel<<<f->n_batch * p.tiles_per_batch, corr::kFftThreads, 0, static_cast<cudaStream_t>(stream)>>>(p);
   CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
+int corr_fstage_set_input(corr_fstage *f, int dtype) {
+  if (!f) return fail(CORR_EINVAL, "corr_fstage_set_input: NULL handle");
+  if (dtype != CORR_CI8 && dtype != CORR_CI4) return fail(CORR_EINVAL, "corr_fstage_set_input: dtype must be CORR_CI8 or CORR_CI4");
+  if (dtype != f->in_dtype) {  // the streaming buffers are sized for the input format
+    cudaFree(f->d_raw[0]);
+    cudaFree(f->d_raw[1]);
+    f->d_raw[0] = f->d_raw[1] = nullptr;
+  }
+  f->in_dtype = dtype;
+  f->in_bytes = static_cast<size_t>(f->n_batch) * f->n_fft * f->n_inputs * (dtype == CORR_CI4 ? 1 : 2);
   return CORR_OK;
 }
 

@@ -28,7 +28,7 @@ constexpr int kFftTile = 32;      // inputs per CTA (one per lane)
 constexpr int kFftThreads = 256;  // 8 warps = the 8 residues n2
 
 struct FftParams {
-  const int8_t *raw;  // [n_batch][128][n_inputs][2]
+  const int8_t *raw;  // [n_batch][128][n_inputs][2] int8 pairs, or [n_batch][128][n_inputs] bytes (4+4-bit mode)
   float2 *spec;       // [n_batch][128][n_inputs]
   int n_batch, n_inputs, tiles_per_batch;
 };
@@ -107,8 +107,10 @@ __device__ __forceinline__ void fft16(float2 (&v)[16]) {
     }
 }
 
-__global__ void __launch_bounds__(kFftThreads, 4)
-fengine_kernel(const FftParams p) {
+// kPacked: the paper's "1-byte mode": one byte per complex sample, low nibble Re, high nibble Im,
+// 4-bit two's complement (DESIGN reading R18) -- half the raw bytes over PCIe and HBM, same transform.
+template <bool kPacked>
+__device__ __forceinline__ void fengine_body(const FftParams &p) {
   __shared__ float2 z[kFftN * kFftTile];  // [n2][k1][lane], 32 KB
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;  // pass 1: n2; pass 2: k1 (and k1 + 8)
@@ -121,20 +123,34 @@ fengine_kernel(const FftParams p) {
 
   // ---- pass 1: unpack (int8 -> float) + 16-point transforms over n1 for residue n2 = w
   {
-    const char2 *src = reinterpret_cast<const char2 *>(p.raw) + (base + w * ni);
-    char2 raw[16];
-#pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) raw[n1] = src[8u * n1 * ni];  // all 16 loads in flight
-    // unpack ("converting to floating-point format") without the quarter-rate I2F: the byte u = x ^ 0x80
-    // placed in the mantissa of 2^23 is the float 8388608 + u; subtracting 8388736 leaves x exactly
     float2 v[16];
+    if (kPacked) {
+      const uint8_t *src = reinterpret_cast<const uint8_t *>(p.raw) + (base + w * ni);
+      uint8_t raw[16];
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) {
-      const uint32_t u = (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].x)) |
-                          (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].y)) << 8)) ^ 0x8080u;
-      const float2 m = make_float2(__uint_as_float(__byte_perm(u, 0x4B000000u, 0x7440)),
-                                   __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441)));
-      v[n1] = csub(m, make_float2(8388736.0f, 8388736.0f));
+      for (int n1 = 0; n1 < 16; ++n1) raw[n1] = src[8u * n1 * ni];  // all 16 loads in flight
+      // a nibble n is the value (n ^ 8) - 8; (n ^ 8) placed in the mantissa of 2^23 is the float 8388608 + (n ^ 8)
+#pragma unroll
+      for (int n1 = 0; n1 < 16; ++n1) {
+        const uint32_t u = static_cast<uint32_t>(raw[n1]) ^ 0x88u;
+        const float2 m = make_float2(__uint_as_float(0x4B000000u | (u & 15u)), __uint_as_float(0x4B000000u | (u >> 4)));
+        v[n1] = csub(m, make_float2(8388616.0f, 8388616.0f));
+      }
+    } else {
+      const char2 *src = reinterpret_cast<const char2 *>(p.raw) + (base + w * ni);
+      char2 raw[16];
+#pragma unroll
+      for (int n1 = 0; n1 < 16; ++n1) raw[n1] = src[8u * n1 * ni];  // all 16 loads in flight
+      // unpack ("converting to floating-point format") without the quarter-rate I2F: the byte u = x ^ 0x80
+      // placed in the mantissa of 2^23 is the float 8388608 + u; subtracting 8388736 leaves x exactly
+#pragma unroll
+      for (int n1 = 0; n1 < 16; ++n1) {
+        const uint32_t u = (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].x)) |
+                            (static_cast<uint32_t>(static_cast<uint8_t>(raw[n1].y)) << 8)) ^ 0x8080u;
+        const float2 m = make_float2(__uint_as_float(__byte_perm(u, 0x4B000000u, 0x7440)),
+                                     __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441)));
+        v[n1] = csub(m, make_float2(8388736.0f, 8388736.0f));
+      }
     }
     fft16(v);
 #pragma unroll
@@ -157,5 +173,8 @@ fengine_kernel(const FftParams p) {
     for (int k2 = 0; k2 < 8; ++k2) dst[16u * k2 * ni] = v[k2];
   }
 }
+
+__global__ void __launch_bounds__(kFftThreads, 4) fengine_kernel(const FftParams p) { fengine_body<false>(p); }
+__global__ void __launch_bounds__(kFftThreads, 4) fengine_ci4_kernel(const FftParams p) { fengine_body<true>(p); }
 
 }  // namespace corr

@@ -131,3 +131,48 @@ def test_stream_run_fx_matches_float64_chain(pkg):
     pkg.corr_destroy(h2)
     pkg.corr_destroy(h)
     pkg.corr_fstage_destroy(f)
+
+
+def raw_voltages_4bit(B, I, seed):
+    """4+4-bit samples: clip(rint(2.5 g), -8, 7), as int8 pairs and packed one byte per sample."""
+    x = corrgen.gauss_i8(B, 128, I, seed, 2.5, 7.0)
+    x[0, :3, 0] = [(-8, 7), (7, -8), (-1, -1)]          # the corners of the 4-bit range
+    x = np.clip(x, -8, 7).astype(np.int8)
+    return x, corrgen.pack_ci4(x)
+
+
+@pytest.mark.parametrize("B,I", [(2, 32), (9, 64), (33, 96)])
+def test_fstage_one_byte_mode(pkg, B, I):
+    """corr_fstage_set_input(CORR_CI4): packed raw voltages give the spectra of the oracle's packed routine -- and
+    bit-identical spectra to the int8 mode on the same samples (the unpack is exact in both)."""
+    x8, xb = raw_voltages_4bit(B, I, seed=60 + B)
+    f = pkg.corr_fstage_create(I, 128, B)
+    s8 = pkg.corr_fstage_run(f, torch.from_numpy(x8).cuda()).cpu().numpy()
+    f.set_input("ci4")
+    assert f.in_bytes == B * 128 * I
+    spec = torch.full((B, 128, I, 2), float("nan"), dtype=torch.float32, device="cuda")
+    pkg.corr_fstage_run(f, torch.from_numpy(xb).cuda(), spec)
+    s4 = spec.cpu().numpy()
+    assert np.array_equal(s4, s8)
+    ref = oracle.fstage_ci4(xb, threads=oracle.host_threads())
+    norm = np.sqrt(np.sum(x8.astype(np.float64) ** 2, axis=(1, 3)))[:, None, :]
+    err = np.hypot(s4[..., 0] - ref[..., 0], s4[..., 1] - ref[..., 1])
+    assert np.max(err / norm) <= 1e-5
+    with pytest.raises(ValueError):
+        pkg.corr_fstage_run(f, torch.from_numpy(x8).cuda())       # wrong size for the packed mode
+    pkg.corr_fstage_destroy(f)
+
+
+def test_stream_run_fx_one_byte_mode(pkg):
+    T, I, n_int = 12, 64, 2
+    pairs = [raw_voltages_4bit(T, I, seed=80 + k) for k in range(n_int)]
+    f = pkg.corr_fstage_create(I, 128, T)
+    f.set_input("ci4")
+    h = pkg.corr_create(I, 128, T, "cf32")
+    d_vis, _ = h.stream_run([torch.from_numpy(xb).pin_memory() for _, xb in pairs], fstage=f)
+    out = d_vis.cpu().numpy()
+    for k, (_, xb) in enumerate(pairs):
+        ref_spec = oracle.fstage_ci4(xb, threads=oracle.host_threads())
+        f32_tolerance_check(out[k], oracle.xengine_cf64(ref_spec, threads=oracle.host_threads()), I, rel=2e-5)
+    pkg.corr_destroy(h)
+    pkg.corr_fstage_destroy(f)
