@@ -131,6 +131,17 @@ def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None):
     out = {"total_s": total, "mean_s": total / steps, "median_s": per[len(per) // 2], "best_s": per[0],
            "launches": steps * h.launches_per_call, "n_buffers": n_buf, "handle": h, "bufs": bufs, "vis": vis}
     if n_buf > 1 and not sampler:
+        # isolated latency of one call (device idle before and after), SURVEY H3
+        lone = []
+        for k in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(stream)
+            h.xengine(bufs[k % n_buf], vis, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            lone.append(e0.elapsed_time(e1) * 1e-3)
+        out["isolated_s"] = sorted(lone)[len(lone) // 2]
         # an integration that fits in L2 is launch-bound when enqueued call by call from Python: the steady
         # state is one CUDA graph of n_buf calls (one per rotating buffer, > 2x L2 in total), replayed
         side = torch.cuda.Stream()
@@ -329,6 +340,7 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     if "graph_s" in r:
         out["timing"] = f"CUDA graph of {r['n_buffers']} calls on rotating buffers, replayed (steady state)"
         out["ms_eager"] = r["median_s"] * 1e3  # call by call from Python: host launch-bound
+        out["ms_isolated"] = r["isolated_s"] * 1e3  # one call on an idle device (launch + kernel latency)
     if "graph4_s" in r:
         out["ms_4streams"] = r["graph4_s"] * 1e3  # the same calls spread over 4 streams of one graph (they overlap)
         out["frac_4streams"] = max(t_a, t_b) / r["graph4_s"]
