@@ -184,6 +184,14 @@ __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bu
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 }  // namespace corr
 
+// ----------------------------------------------------------------------------- programmatic dependent launch
+namespace corr {
+// let the next kernel of the stream start its prologue now (it still waits for this grid before touching memory)
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// wait until the preceding grid of the stream has completed and its writes are visible
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+}  // namespace corr
+
 // ----------------------------------------------------------------------------- CTA pairs (cta_group::2)
 namespace corr {
 __device__ __forceinline__ uint32_t cluster_ctarank() {

@@ -47,6 +47,9 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
   uint64_t *raw_empty = raw_full + kMaxStages;
   uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(raw_empty + kMaxStages);
 
+  // programmatic dependent launch (single-CTA kernels): the next call's launch, barrier set-up and TMEM allocation may
+  // overlap this call's tail; every role that touches global memory waits for the preceding grid first
+  if (!kPair) griddep_launch_dependents();
   const int probe = kProbe ? p.probe : 0;  // diagnostics compile away in the production instantiation
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -87,6 +90,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     const int pw = (warp == kProducerWarp) ? 0 : 1;
     int iter = 0;
     if (elect_one() && !(probe & 8)) {
+      if (!kPair) griddep_wait();  // d_in may have been written by the preceding kernel of the stream
       const uint64_t pol = policy_evict_normal();
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
@@ -266,6 +270,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     }
   } else if (warp < kEpiWarps && !(probe & 4)) {
     // ===================================================================== epilogue
+    if (!kPair) griddep_wait();  // d_vis may still be written (or read) by the preceding kernel of the stream
     const int ew = warp & 3;         // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
     constexpr int kShift = kPacked ? 8 : 0;

@@ -236,3 +236,39 @@ def test_cf32_n64_paths_within_tolerance(pkg, monkeypatch, generic, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c5"], n_inputs=64, n_chan=C, n_time=T)
     x = w.generate()
     f32_tolerance_check(run_cf32(pkg, x), oracle.xengine_cf32(x, threads=_threads()), 64)
+
+
+def test_ci8_cuda_graph_with_dependent_launches(pkg):
+    """Calls captured into a CUDA graph launch programmatically (the next kernel may start while the preceding one
+    drains): results must not depend on it -- the same d_vis written by consecutive calls (write after write), and an
+    input produced by the preceding kernel of the stream (standalone corner turn -> X-engine)."""
+    w = corrgen.scaled(corrgen.CONFIGS["c1"], n_chan=24, n_time=300)
+    xs = [w.generate(integration=k) for k in range(3)]
+    refs = [oracle.xengine_ci8(x, threads=_threads()) for x in xs]
+    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, "ci8")
+    ht = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, "ci8")
+    ht.set_turn(pkg.CORR_TURN_STANDALONE)
+    d = [torch.from_numpy(x).cuda() for x in xs]
+    va, vb, vc = h.empty_vis(), h.empty_vis(), h.empty_vis()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        h.xengine(d[0], va, s)
+        ht.xengine(d[2], vc, s)   # warm-up outside the capture (allocates the turn scratch)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            h.xengine(d[0], va, s)
+            h.xengine(d[1], va, s)     # same output buffer as the call before
+            h.xengine(d[2], vb, s)
+            ht.xengine(d[0], vc, s)    # corner-turn kernel, then the X-engine on its output
+        for buf in (va, vb, vc):
+            buf.fill_(-0x55555555)
+        g.replay()
+        g.replay()
+        torch.cuda.synchronize()
+    assert np.array_equal(va.cpu().numpy(), refs[1])
+    assert np.array_equal(vb.cpu().numpy(), refs[2])
+    assert np.array_equal(vc.cpu().numpy(), refs[0])
+    del g
+    pkg.corr_destroy(h)
+    pkg.corr_destroy(ht)
