@@ -2,12 +2,12 @@
 
 TEST INFRASTRUCTURE: only ``tests/``, ``__graft_entry__.smoke()`` and
 ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this
-package.  The product package never does (tests/test_independence.py checks).
+package.  The product package never does (tests/test_abi_cpu.py::test_product_and_oracle_are_independent checks).
 
 All arithmetic is in ``xcorr_oracle.c`` (read its header for the passages it
 follows: PAPER.md:47, :53, :84, :107, :115).  This file only marshals numpy
 arrays.  Parity status: every function below is pinned by
-``tests/test_oracle_pins.py`` (P1-P9, P11-P12 for the 4-bit mode, tests/golden/) or, for the F-stage
+``tests/test_oracle_pins.py`` (P1-P9, P11-P12 for the 4-bit mode, P14 for the int64 accumulation, tests/golden/) or, for the F-stage
 (``fstage_oracle.c``), ``tests/test_oracle_fstage_pins.py`` (F1-F7); none is "parity unpinned".
 """
 from __future__ import annotations
@@ -53,6 +53,9 @@ def _load():
         _lib.oracle_readout_i32.argtypes = [P, L, ctypes.c_double, P]
         _lib.oracle_readout_f64.argtypes = [P, L, ctypes.c_double, P]
         _lib.oracle_readout_i32.restype = _lib.oracle_readout_f64.restype = None
+        _lib.oracle_xengine_ci8_wide.argtypes = [P, L, L, L, L, L, P, I]
+        _lib.oracle_readout_i64.argtypes = [P, L, ctypes.c_double, P]
+        _lib.oracle_readout_i64.restype = None
         _lib.oracle_full_matrix_ci8.argtypes = [P, L, L, L, L, P]
         _lib.oracle_full_matrix_cf32.argtypes = [P, L, L, L, L, P]
         _lib.oracle_one_visibility_ci8.argtypes = [P, L, L, L, L, L, L, P]
@@ -87,6 +90,18 @@ def xengine_ci8(x, c_begin=0, c_end=None, threads=1):
     return vis
 
 
+def xengine_ci8_wide(x, c_begin=0, c_end=None, threads=1):
+    """x: int8 [T][C][N][2], any T -> int64 [c_end-c_begin][N(N+1)/2][2]: the sums of a long accumulation
+    (PAPER.md:84, :125), never refused for overflow."""
+    x, T, C, N = _check_cube(x, np.int8)
+    c_end = C if c_end is None else c_end
+    vis = np.empty((c_end - c_begin, N * (N + 1) // 2, 2), dtype=np.int64)
+    rc = _load().oracle_xengine_ci8_wide(x.ctypes.data, T, C, N, c_begin, c_end, vis.ctypes.data, threads)
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return vis
+
+
 def unpack_ci4(byte):
     """(re, im) of one packed 4+4-bit sample (reading R18: low nibble Re, high nibble Im, two's complement)."""
     re, im = ctypes.c_int(), ctypes.c_int()
@@ -114,10 +129,12 @@ def readout(vis, count):
     out = np.empty(vis.shape, dtype=np.float64)
     if vis.dtype == np.int32:
         _load().oracle_readout_i32(vis.ctypes.data, vis.size, float(count), out.ctypes.data)
+    elif vis.dtype == np.int64:
+        _load().oracle_readout_i64(vis.ctypes.data, vis.size, float(count), out.ctypes.data)
     elif vis.dtype == np.float64:
         _load().oracle_readout_f64(vis.ctypes.data, vis.size, float(count), out.ctypes.data)
     else:
-        raise ValueError("readout expects int32 or float64 sums")
+        raise ValueError("readout expects int32, int64 or float64 sums")
     return out
 
 

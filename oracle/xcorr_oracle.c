@@ -260,3 +260,40 @@ void oracle_readout_f64(const double *vis, long n_scalars, double count, double 
 {
     for (long k = 0; k < n_scalars; ++k) out[k] = vis[k] / count;
 }
+
+/*
+ * Long accumulations (the accumulators are read "after a specified time, usually a few
+ * seconds"; every batch of spectra is ADDED to the persistent accumulators).  The
+ * definition is the same sum over ALL samples of all batches; only the output word is wider: int64, so
+ * that no int8 input can overflow for any realistic T (|V| <= T * 2 * 128^2 < 2^63 for T < 2.8e14).
+ * Same five loops as oracle_xengine_ci8, without the int32 check.
+ */
+int oracle_xengine_ci8_wide(const int8_t *x, long n_time, long n_chan, long n_inputs,
+                            long c_begin, long c_end, int64_t *vis, int threads)
+{
+    const long nb = n_inputs * (n_inputs + 1) / 2;
+    (void)threads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads > 1 ? threads : 1)
+    for (long c = c_begin; c < c_end; ++c) {
+        int64_t *acc = vis + 2 * nb * (c - c_begin);
+        memset(acc, 0, (size_t)(2 * nb) * sizeof(int64_t));
+        for (long t = 0; t < n_time; ++t) {
+            const int8_t *xt = x + 2 * ((t * n_chan + c) * n_inputs);
+            long b = 0;
+            for (long i = 0; i < n_inputs; ++i) {
+                const int64_t a_i = xt[2 * i], b_i = xt[2 * i + 1];
+                for (long j = 0; j <= i; ++j, ++b) {
+                    const int64_t a_j = xt[2 * j], b_j = xt[2 * j + 1];
+                    acc[2 * b] += a_i * a_j + b_i * b_j;     /* Re x_i conj(x_j) */
+                    acc[2 * b + 1] += b_i * a_j - a_i * b_j; /* Im x_i conj(x_j) */
+                }
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+void oracle_readout_i64(const int64_t *vis, long n_scalars, double count, double *out)
+{
+    for (long k = 0; k < n_scalars; ++k) out[k] = (double)vis[k] / count;
+}

@@ -319,3 +319,55 @@ def test_p10_tone_phase_statistics():
                 v = complex(*vis[c, tri_index(i, j)])
                 d = np.angle(v * np.exp(-1j * (phi[c, i] - phi[c, j])))
                 assert abs(d) < 0.15
+
+
+# ----------------------------------------------------------------------------- P14: int64 accumulation
+# (PAPER.md:84 "after a specified time, usually a few seconds"; :125, :166: batches are ADDED to the accumulators)
+
+def test_p14_wide_closed_form_beyond_int32():
+    """Constant full-scale input for T = 70000 samples: V_ij = T x_i conj(x_j) = 70000 * 2 * 127^2 = 2.26e9 > 2^31 - 1.
+    The int32 routine must refuse it, the int64 routine must give the closed form exactly."""
+    T = 70000
+    x = np.empty((T, 1, 2, 2), np.int8)
+    x[:, 0, 0] = (127, -127)
+    x[:, 0, 1] = (-128, 127)
+    with pytest.raises(oracle.OracleOverflow):
+        oracle.xengine_ci8(x)
+    v = oracle.xengine_ci8_wide(x)
+    assert v.dtype == np.int64
+    z = [127 - 127j, -128 + 127j]
+    want = {(0, 0): T * z[0] * np.conj(z[0]), (1, 0): T * z[1] * np.conj(z[0]), (1, 1): T * z[1] * np.conj(z[1])}
+    for (i, j), w in want.items():
+        assert v[0, tri_index(i, j), 0] == int(round(w.real)) and v[0, tri_index(i, j), 1] == int(round(w.imag)), (i, j)
+    assert v[0, tri_index(0, 0), 0] > 2**31 - 1
+
+
+def test_p14_wide_equals_int32_routine_and_sums_of_batches():
+    """Where the sums fit, the int64 routine equals the (pinned) int32 routine; and it is the sum of the batches'
+    int32 results -- what an accumulating correlator adds up (linearity, P4)."""
+    x = rand_ci8(90, 3, 6, 21)
+    wide = oracle.xengine_ci8_wide(x, threads=2)
+    assert np.array_equal(wide, oracle.xengine_ci8(x).astype(np.int64))
+    parts = sum(oracle.xengine_ci8(x[a:b]).astype(np.int64) for a, b in ((0, 17), (17, 60), (60, 90)))
+    assert np.array_equal(wide, parts)
+    sub = oracle.xengine_ci8_wide(x, 1, 3)
+    assert np.array_equal(sub, wide[1:3])
+
+
+def test_p14_wide_against_numpy_hermitian_product():
+    x = rand_ci8(40, 2, 5, 22)
+    wide = oracle.xengine_ci8_wide(x)
+    z = as_complex(x)
+    for c in range(2):
+        X = z[:, c, :].T                                   # [N][T]
+        V = X @ X.conj().T
+        for i in range(5):
+            for j in range(i + 1):
+                assert wide[c, tri_index(i, j), 0] == int(round(V[i, j].real))
+                assert wide[c, tri_index(i, j), 1] == int(round(V[i, j].imag))
+
+
+def test_p14_readout_of_int64_sums():
+    v = np.array([[[2**40 + 4, -(2**35)]]], dtype=np.int64)
+    out = oracle.readout(v, 4)
+    assert out[0, 0, 0] == 2.0**38 + 1.0 and out[0, 0, 1] == -(2.0**33)
