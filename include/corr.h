@@ -55,7 +55,7 @@ enum { CORR_TURN_FUSED = 0,     /* the TMA box load of the CMAC kernel is the co
  *   n_chan   C   : >= 1
  *   n_time   T   : >= 1; for CORR_CI8 also T <= 65535 so that no int8 input can
  *                  overflow int32 (|V| <= T*2*128^2; reading R6)
- *   dtype        : CORR_CI8 or CORR_CF32
+ *   dtype        : CORR_CI8, CORR_CF32 or CORR_CI4 (T <= 65535 for CORR_CI4 as well)
  * Returns NULL on failure; corr_last_error()/corr_last_status() say why
  * (CORR_EINVAL, CORR_EUNSUPPORTED shape, CORR_EARCH not sm_100, CORR_EALLOC, CORR_ECUDA).
  * The handle owns its device workspaces (tile schedule, corner-turn scratch) until
@@ -100,9 +100,30 @@ int corr_set_turn(corr_handle *h, int mode);
 /*
  * corr_set_accumulate -- accumulate mode (each batch's products are ADDED to the
  * accumulators).  on != 0: corr_xengine adds the sums of its integration to d_vis instead of overwriting
- * it (the caller zeroes d_vis before the first call; integer sums stay exact as long as they fit int32).
+ * it; the caller zeroes d_vis and calls corr_set_accumulate(h, 1) at the START of every accumulation --
+ * the call resets the handle's update counter.  int32 accumulators cannot hold an arbitrary number of
+ * batches: corr_xengine returns CORR_EUNSUPPORTED (and adds nothing) once another batch could overflow
+ * them for SOME input, i.e. when (count + 1) * T * 2 * 128^2 >= 2^31 (CORR_CI8) or
+ * (count + 1) * T * 2 * 8^2 >= 2^31 (CORR_CI4); CORR_CF32 has no such bound.  For longer accumulations
+ * use corr_accumulate_wide.  corr_accumulate_count returns the number of batches added so far.
  */
 int corr_set_accumulate(corr_handle *h, int on);
+long long corr_accumulate_count(const corr_handle *h);
+
+/*
+ * corr_accumulate_wide -- one batch added into accumulators twice as wide (read out "after a
+ * specified time, usually a few seconds"): the integration of d_in is computed into a
+ * handle-owned buffer (corr_vis_bytes) and then folded, acc[k] += vis[k], into
+ *   d_acc : device, [n_chan][N_I(N_I+1)/2] (int64 re, int64 im) for CORR_CI8 / CORR_CI4 -- exact for any
+ *           number of batches -- or (double re, double im) for CORR_CF32; corr_acc_bytes(h) bytes,
+ *           16-byte aligned, zeroed by the caller before the first batch.
+ * Independent of corr_set_accumulate.  Asynchronous on `stream`.  Returns CORR_OK, CORR_EINVAL, CORR_EALLOC
+ * or CORR_ECUDA.  corr_normalize_wide is the read-out of d_acc (count = samples accumulated) into
+ * (float re, float im), d_out of corr_vis_bytes(h) bytes.
+ */
+int corr_accumulate_wide(corr_handle *h, const void *d_in, void *d_acc, void *stream);
+int corr_normalize_wide(corr_handle *h, const void *d_acc, double count, void *d_out, void *stream);
+size_t corr_acc_bytes(const corr_handle *h); /* 2 * corr_vis_bytes */
 
 /*
  * corr_normalize -- read-out (the accumulators are "divided by the number of times they were
@@ -113,23 +134,43 @@ int corr_set_accumulate(corr_handle *h, int on);
 int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out, void *stream);
 
 /*
- * corr_set_probe -- DIAGNOSTICS ONLY (results are garbage while a probe is on): switches engines of the CI8
- * kernel off so that the others can be timed alone.  Bit mask: 1 = skip the MMAs, 2 = skip the TMA loads
- * (producer only hand-shakes), 4 = no epilogue, 8 = no producer and no stage hand-shake at all, 16 = epilogue
- * without its global stores; 0 = normal (the production instantiation has none of this code).  Used by the
- * roofline study in DESIGN.md section 7, never by tests of results.
+ * corr_xengine_batch -- n whole integrations in ONE launch ("it is most efficient to transfer
+ * and process large batches of data per call"; 32 blocks of spectra per GPU call).  An
+ * integration too small to fill the chip (config 1: 8 MB) costs a launch, a pipeline fill and one exposed
+ * DRAM round trip per call; here the tile schedule spans all n inputs, so every SM streams for the whole call.
+ *   d_in  : HOST array of n device pointers, each as corr_xengine's d_in
+ *   d_vis : HOST array of n device pointers, each as corr_xengine's d_vis (distinct buffers)
+ *   n     : >= 1; more than 64 integrations are issued as several launches of <= 64
+ * Same result as n corr_xengine calls (bit-exact for CI8).  The single-launch path covers CORR_CI8 shapes
+ * that run on single CTAs (N_I <= 64, and 128 <= N_I < 512 unless the integration is long); every other
+ * case (CTA-pair plans, CORR_CI4, CORR_CF32, the standalone corner turn, accumulate mode) falls back to n
+ * ordinary calls on `stream`.  Returns as corr_xengine.
  */
-int corr_set_probe(corr_handle *h, int mode);
+int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_vis, int n, void *stream);
 
 /*
- * corr_probe_mma -- measures the tcgen05.mma.kind::i8 issue rate on the current device (the int8
- * tensor peak the roofline needs; it is not in MEASURED_PEAKS.json).  M in {64,128}, N multiple of
- * 16 <= 256, K = 32; mn_major = 1 for the operand layout the fused corner turn produces, 0 for
- * K-major (add 2 for pseudo-random instead of zero operand bytes).  out[0] = kernel ms, out[1] = SM
- * cycles per MMA, out[2] = dense TOP/s over all SMs, out[3] = effective SM MHz during the loop.
- * No global-memory traffic; shared-memory operands are zeros.
+ * corr_set_chan_window -- channel-sharded use ("The products are formed
+ * independently for each frequency channel"): the handle (created with n_chan = the window's
+ * width) reads channels chan0 .. chan0 + n_chan - 1 of a buffer d_in[n_time][n_chan_total][n_inputs] IN
+ * PLACE -- no copy, the TMA tensor map / the float kernels take the full row as their time stride -- and
+ * writes its own [n_chan][N_I(N_I+1)/2] block to d_vis.  After the call corr_in_bytes(h) is the size of
+ * the FULL buffer.  n_chan_total >= chan0 + n_chan, chan0 >= 0; (n_chan_total, 0) with n_chan_total ==
+ * n_chan restores the default.  CORR_EINVAL otherwise.  All dtypes, both corner-turn realisations.
  */
-int corr_probe_mma(int m, int n, int mn_major, int iters, double *out);
+int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
+
+/*
+ * corr_set_option -- plan knobs for A/B measurements and tests.  Each call re-plans
+ * the handle; the defaults are what corr_create chose.  CORR_EINVAL for an unknown key or a value out of range.
+ */
+enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
+                                   panels per work item and `slices` (1..64) time slices; 0 = automatic       */
+       CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
+       CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default)                                     */
+       CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
+       CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
+       CORR_OPT_PDL = 6         /* 0: never launch programmatically inside a stream capture; 1 (default)      */ };
+int corr_set_option(corr_handle *h, int key, int value);
 
 /*
  * corr_corner_turn -- the standalone corner-turn kernel, CI8 or CF32:

@@ -1,0 +1,48 @@
+/*
+ * corr_diag.h -- DIAGNOSTICS of the B200 X-engine library.  Not part of the product ABI (include/corr.h):
+ * these entry points exist only in libcorr_diag.so, the same sources compiled with -DCORR_DIAG, which also
+ * carries a second, probe-instrumented instantiation of the int8 kernels.  The product library libcorr.so
+ * has one instantiation of each hot kernel and none of this.
+ *
+ * Used by bench.py for the roofline denominators MEASURED_PEAKS.json does not hold (int8 tensor rate, FP32
+ * FMA rate) and by the where-the-time-goes study of DESIGN.md section 7.  Results computed while a probe
+ * mode is on are garbage by design; no test of results uses them.
+ */
+#ifndef CORR_DIAG_H_
+#define CORR_DIAG_H_
+
+#include "corr.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/*
+ * corr_set_probe -- switches engines of the CI8 kernel off so that the others can be timed alone.  Bit
+ * mask: 1 = skip the MMAs, 2 = skip the TMA loads (producer only hand-shakes), 4 = no epilogue, 8 = no
+ * producer and no stage hand-shake at all, 16 = epilogue without its global stores; 0 = normal.
+ */
+int corr_set_probe(corr_handle *h, int mode);
+
+/*
+ * corr_probe_mma -- tcgen05.mma.kind::i8 issue rate on the current device (the int8 tensor peak of the
+ * roofline).  M in {64,128}, N multiple of 16 <= 256, K = 32; mn_major = 1 for the operand layout the
+ * fused corner turn produces, 0 for K-major (add 2 for pseudo-random instead of zero operand bytes).
+ * out[0] = kernel ms, out[1] = SM cycles per MMA, out[2] = dense TOP/s over all SMs, out[3] = effective
+ * SM MHz during the loop.  No global-memory traffic.
+ */
+int corr_probe_mma(int m, int n, int mn_major, int iters, double *out);
+
+/*
+ * corr_probe_ffma -- FP32 FMA issue rate on the current device (the "alu" roofline denominator of the
+ * float X-engine): 2 CTAs x 512 threads per SM, 16 independent register-resident FMA chains per thread,
+ * `iters` rounds; packed = 0: scalar fma.rn.f32, 1: fma.rn.f32x2 (what xengine_f32_n64_kernel issues).
+ * out[0] = kernel ms, out[1] = TFLOP/s over all SMs (2 flops per FMA, over the loop itself),
+ * out[2] = effective SM MHz during the loop.
+ */
+int corr_probe_ffma(int packed, int iters, double *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CORR_DIAG_H_ */

@@ -15,13 +15,20 @@ from . import build as _build
 CORR_CI8, CORR_CF32, CORR_CI4 = 0, 1, 2
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
 CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
+CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL = 1, 2, 3, 4, 5, 6
 
+# include/corr.h (the product ABI, libcorr.so)
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
-           "corr_corner_turn", "corr_stream_run", "corr_set_probe", "corr_probe_mma", "corr_set_accumulate", "corr_normalize",
+           "corr_corner_turn", "corr_stream_run", "corr_set_accumulate", "corr_accumulate_count", "corr_normalize",
+           "corr_accumulate_wide", "corr_normalize_wide", "corr_acc_bytes", "corr_xengine_batch", "corr_set_chan_window",
+           "corr_set_option",
            "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx", "corr_fstage_set_input")
+# include/corr_diag.h (diagnostics, libcorr_diag.so only)
+DIAG_EXPORTS = ("corr_set_probe", "corr_probe_mma", "corr_probe_ffma")
 
 _lib = None
+_diag = False
 
 
 class CorrError(RuntimeError):
@@ -30,47 +37,88 @@ class CorrError(RuntimeError):
         self.status = status
 
 
+def use_diag_build():
+    """Route the whole binding through libcorr_diag.so (the -DCORR_DIAG build: include/corr_diag.h), for the
+    where-the-time-goes study.  Must be called before the first lib()."""
+    global _diag
+    if _lib is not None and not _diag:
+        raise RuntimeError("use_diag_build() must come before the library is first loaded")
+    _diag = True
+
+
+def _bind(path, diag):
+    L = ctypes.CDLL(path)
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    L.corr_create.restype, L.corr_create.argtypes = vp, [ci, ci, ci, ci]
+    L.corr_xengine.restype, L.corr_xengine.argtypes = ci, [vp, vp, vp, vp]
+    L.corr_destroy.restype, L.corr_destroy.argtypes = ci, [vp]
+    L.corr_last_error.restype, L.corr_last_error.argtypes = ctypes.c_char_p, []
+    L.corr_last_status.restype, L.corr_last_status.argtypes = ci, []
+    L.corr_in_bytes.restype, L.corr_in_bytes.argtypes = ctypes.c_size_t, [vp]
+    L.corr_vis_bytes.restype, L.corr_vis_bytes.argtypes = ctypes.c_size_t, [vp]
+    L.corr_launches_per_call.restype, L.corr_launches_per_call.argtypes = ci, [vp]
+    L.corr_set_turn.restype, L.corr_set_turn.argtypes = ci, [vp, ci]
+    L.corr_set_accumulate.restype, L.corr_set_accumulate.argtypes = ci, [vp, ci]
+    L.corr_accumulate_count.restype, L.corr_accumulate_count.argtypes = ctypes.c_longlong, [vp]
+    L.corr_normalize.restype = ci
+    L.corr_normalize.argtypes = [vp, vp, ctypes.c_double, vp, vp]
+    L.corr_normalize_wide.restype = ci
+    L.corr_normalize_wide.argtypes = [vp, vp, ctypes.c_double, vp, vp]
+    L.corr_accumulate_wide.restype, L.corr_accumulate_wide.argtypes = ci, [vp, vp, vp, vp]
+    L.corr_acc_bytes.restype, L.corr_acc_bytes.argtypes = ctypes.c_size_t, [vp]
+    L.corr_xengine_batch.restype = ci
+    L.corr_xengine_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ci, vp]
+    L.corr_set_chan_window.restype, L.corr_set_chan_window.argtypes = ci, [vp, ci, ci]
+    L.corr_set_option.restype, L.corr_set_option.argtypes = ci, [vp, ci, ci]
+    if diag:
+        L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
+        L.corr_probe_mma.restype = ci
+        L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
+        L.corr_probe_ffma.restype = ci
+        L.corr_probe_ffma.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
+    L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
+    L.corr_fstage_create.restype, L.corr_fstage_create.argtypes = vp, [ci, ci, ci]
+    L.corr_fstage_run.restype, L.corr_fstage_run.argtypes = ci, [vp, vp, vp, vp]
+    L.corr_fstage_destroy.restype, L.corr_fstage_destroy.argtypes = ci, [vp]
+    L.corr_fstage_set_input.restype, L.corr_fstage_set_input.argtypes = ci, [vp, ci]
+    L.corr_fstage_in_bytes.restype, L.corr_fstage_in_bytes.argtypes = ctypes.c_size_t, [vp]
+    L.corr_fstage_out_bytes.restype, L.corr_fstage_out_bytes.argtypes = ctypes.c_size_t, [vp]
+    L.corr_stream_run_fx.restype = ci
+    L.corr_stream_run_fx.argtypes = [vp, vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
+    L.corr_stream_run.restype = ci
+    L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
+    return L
+
+
 def lib():
     """Load libcorr.so (building it in-tree first if it is stale and nvcc is present)."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if _build.stale():
-            path = _build.build()
-        L = ctypes.CDLL(path)
-        vp, ci = ctypes.c_void_p, ctypes.c_int
-        L.corr_create.restype, L.corr_create.argtypes = vp, [ci, ci, ci, ci]
-        L.corr_xengine.restype, L.corr_xengine.argtypes = ci, [vp, vp, vp, vp]
-        L.corr_destroy.restype, L.corr_destroy.argtypes = ci, [vp]
-        L.corr_last_error.restype, L.corr_last_error.argtypes = ctypes.c_char_p, []
-        L.corr_last_status.restype, L.corr_last_status.argtypes = ci, []
-        L.corr_in_bytes.restype, L.corr_in_bytes.argtypes = ctypes.c_size_t, [vp]
-        L.corr_vis_bytes.restype, L.corr_vis_bytes.argtypes = ctypes.c_size_t, [vp]
-        L.corr_launches_per_call.restype, L.corr_launches_per_call.argtypes = ci, [vp]
-        L.corr_set_turn.restype, L.corr_set_turn.argtypes = ci, [vp, ci]
-        L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
-        L.corr_set_accumulate.restype, L.corr_set_accumulate.argtypes = ci, [vp, ci]
-        L.corr_normalize.restype = ci
-        L.corr_normalize.argtypes = [vp, vp, ctypes.c_double, vp, vp]
-        L.corr_probe_mma.restype = ci
-        L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
-        L.corr_corner_turn.restype, L.corr_corner_turn.argtypes = ci, [vp, vp, vp, vp]
-        L.corr_fstage_create.restype, L.corr_fstage_create.argtypes = vp, [ci, ci, ci]
-        L.corr_fstage_run.restype, L.corr_fstage_run.argtypes = ci, [vp, vp, vp, vp]
-        L.corr_fstage_destroy.restype, L.corr_fstage_destroy.argtypes = ci, [vp]
-        L.corr_fstage_set_input.restype, L.corr_fstage_set_input.argtypes = ci, [vp, ci]
-        L.corr_fstage_in_bytes.restype, L.corr_fstage_in_bytes.argtypes = ctypes.c_size_t, [vp]
-        L.corr_fstage_out_bytes.restype, L.corr_fstage_out_bytes.argtypes = ctypes.c_size_t, [vp]
-        L.corr_stream_run_fx.restype = ci
-        L.corr_stream_run_fx.argtypes = [vp, vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
-        L.corr_stream_run.restype = ci
-        L.corr_stream_run.argtypes = [vp, ctypes.POINTER(vp), ci, vp, ctypes.POINTER(ctypes.c_double)]
-        _lib = L
+        path = _build.LIB_DIAG if _diag else _build.LIB
+        if _build.stale(_diag):
+            path = _build.build(diag=_diag)
+        _lib = _bind(path, _diag)
     return _lib
 
 
-def _raise():
-    L = lib()
+_diag_lib = None
+
+
+def diag_lib():
+    """libcorr_diag.so (include/corr_diag.h): peak probes and engine switches.  Diagnostics only."""
+    global _diag_lib
+    if _diag:
+        return lib()
+    if _diag_lib is None:
+        path = _build.LIB_DIAG
+        if _build.stale(True):
+            path = _build.build(diag=True)
+        _diag_lib = _bind(path, True)
+    return _diag_lib
+
+
+def _raise(L=None):
+    L = L or lib()
     raise CorrError(L.corr_last_status(), L.corr_last_error().decode())
 
 
@@ -110,10 +158,69 @@ class Correlator:
         if lib().corr_set_turn(self._h, mode) != CORR_OK:
             _raise()
 
+    # -- corr_set_option / corr_set_chan_window
+    def set_option(self, key, value):
+        if lib().corr_set_option(self._h, key, value) != CORR_OK:
+            _raise()
+
+    def set_chan_window(self, n_chan_total, chan0):
+        """Read channels chan0 .. chan0 + n_chan - 1 of a [T][n_chan_total][N] buffer in place."""
+        if lib().corr_set_chan_window(self._h, n_chan_total, chan0) != CORR_OK:
+            _raise()
+        self.in_bytes = lib().corr_in_bytes(self._h)
+
+    def set_probe(self, mode):
+        """Diagnostics build only (use_diag_build())."""
+        if lib().corr_set_probe(self._h, mode) != CORR_OK:
+            _raise()
+
     # -- corr_set_accumulate / corr_normalize
     def set_accumulate(self, on=True):
         if lib().corr_set_accumulate(self._h, 1 if on else 0) != CORR_OK:
             _raise()
+
+    @property
+    def accumulate_count(self):
+        return lib().corr_accumulate_count(self._h)
+
+    # -- corr_accumulate_wide / corr_normalize_wide
+    def empty_acc(self):
+        """Zeroed wide accumulators [C][N(N+1)/2][2]: int64 (CI8, CI4) or float64 (CF32)."""
+        import torch
+        dt = torch.float64 if self.dtype == CORR_CF32 else torch.int64
+        return torch.zeros((self.n_chan, self.n_baselines, 2), dtype=dt, device="cuda")
+
+    def accumulate_wide(self, d_in, d_acc, stream=None):
+        self._check_in(d_in)
+        if not d_acc.is_cuda or not d_acc.is_contiguous() or d_acc.numel() * d_acc.element_size() != 2 * self.vis_bytes:
+            raise ValueError(f"d_acc must be a contiguous CUDA tensor of {2 * self.vis_bytes} bytes")
+        if lib().corr_accumulate_wide(self._h, d_in.data_ptr(), d_acc.data_ptr(), _stream_ptr(stream)) != CORR_OK:
+            _raise()
+        return d_acc
+
+    def normalize_wide(self, d_acc, count, d_out=None, stream=None):
+        import torch
+        if d_out is None:
+            d_out = torch.empty(d_acc.shape, dtype=torch.float32, device="cuda")
+        if lib().corr_normalize_wide(self._h, d_acc.data_ptr(), float(count), d_out.data_ptr(), _stream_ptr(stream)) != CORR_OK:
+            _raise()
+        return d_out
+
+    # -- corr_xengine_batch
+    def xengine_batch(self, d_in_list, d_vis_list=None, stream=None):
+        """n integrations in one launch: lists of CUDA tensors, as xengine()."""
+        n = len(d_in_list)
+        if d_vis_list is None:
+            d_vis_list = [self.empty_vis() for _ in range(n)]
+        for d_in, d_vis in zip(d_in_list, d_vis_list):
+            self._check_in(d_in)
+            if not d_vis.is_cuda or not d_vis.is_contiguous() or d_vis.numel() * d_vis.element_size() != self.vis_bytes:
+                raise ValueError(f"every d_vis must be a contiguous CUDA tensor of {self.vis_bytes} bytes")
+        pin = (ctypes.c_void_p * n)(*[t.data_ptr() for t in d_in_list])
+        pout = (ctypes.c_void_p * n)(*[t.data_ptr() for t in d_vis_list])
+        if lib().corr_xengine_batch(self._h, pin, pout, n, _stream_ptr(stream)) != CORR_OK:
+            _raise()
+        return d_vis_list
 
     def normalize(self, d_vis, count, d_out=None, stream=None):
         """d_vis (raw sums) / count -> float32 [C][N(N+1)/2][2] (PAPER.md:84 read-out)."""
@@ -183,11 +290,21 @@ class Correlator:
 
 
 def probe_mma(m=128, n=256, mn_major=True, iters=4096, random_fill=False):
-    """tcgen05 int8 MMA issue-rate probe (see corr_probe_mma)."""
+    """tcgen05 int8 MMA issue-rate probe (corr_probe_mma, include/corr_diag.h; runs in libcorr_diag.so)."""
     out = (ctypes.c_double * 4)()
-    if lib().corr_probe_mma(m, n, (1 if mn_major else 0) | (2 if random_fill else 0), iters, out) != CORR_OK:
-        _raise()
+    L = diag_lib()
+    if L.corr_probe_mma(m, n, (1 if mn_major else 0) | (2 if random_fill else 0), iters, out) != CORR_OK:
+        _raise(L)
     return {"ms": out[0], "cycles_per_mma": out[1], "tops": out[2], "sm_mhz": out[3]}
+
+
+def probe_ffma(packed=True, iters=8192):
+    """FP32 FMA issue-rate probe (corr_probe_ffma, include/corr_diag.h; runs in libcorr_diag.so)."""
+    out = (ctypes.c_double * 3)()
+    L = diag_lib()
+    if L.corr_probe_ffma(1 if packed else 0, iters, out) != CORR_OK:
+        _raise(L)
+    return {"ms": out[0], "tflops": out[1], "sm_mhz": out[2]}
 
 
 class FStage:
@@ -226,6 +343,8 @@ class FStage:
             lib().corr_fstage_destroy(self._f)
             self._f = None
 
+    __del__ = destroy
+
 
 def corr_fstage_create(n_inputs, n_fft, n_batch):
     return FStage(n_inputs, n_fft, n_batch)
@@ -245,6 +364,10 @@ def corr_create(n_inputs, n_chan, n_time, dtype):
 
 def corr_xengine(handle, d_in, d_vis=None, stream=None):
     return handle.xengine(d_in, d_vis, stream)
+
+
+def corr_xengine_batch(handle, d_in_list, d_vis_list=None, stream=None):
+    return handle.xengine_batch(d_in_list, d_vis_list, stream)
 
 
 def corr_destroy(handle):

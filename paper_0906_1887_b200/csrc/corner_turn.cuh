@@ -23,12 +23,16 @@ struct TurnParams {
   int n_groups;  // G
   int wc;        // W / 16: 16-byte chunks per (t, g) row
   int tt, gg;    // tile extents (tt * gg * wc * 16 <= kTurnTileBytes)
+  int g_tiles;   // ceil(G / gg): blockIdx.x = time tile * g_tiles + group tile (1-D grid: no 65535 limit on either)
+  long long in_row_chunks;  // 16-byte chunks per time row of `in` (the full channel axis of a windowed handle)
+  long long in_off_chunks;  // first chunk of group 0 within a time row of `in`
 };
 
 __global__ void __launch_bounds__(kTurnThreads) corner_turn_kernel(const TurnParams p) {
   __shared__ uint4 tile[kTurnTileBytes / 16];
-  const int t0 = blockIdx.y * p.tt;
-  const int g0 = blockIdx.x * p.gg;
+  const int t_tile = blockIdx.x / p.g_tiles;
+  const int t0 = t_tile * p.tt;
+  const int g0 = (blockIdx.x - t_tile * p.g_tiles) * p.gg;
   const int tt = min(p.tt, p.n_time - t0);
   const int gg = min(p.gg, p.n_groups - g0);
   const int row_chunks = gg * p.wc;  // contiguous 16-byte chunks per time row of this tile
@@ -36,7 +40,7 @@ __global__ void __launch_bounds__(kTurnThreads) corner_turn_kernel(const TurnPar
   // load: chunk fastest, then group, then time  (global reads contiguous per time row)
   for (int idx = threadIdx.x; idx < n; idx += kTurnThreads) {
     const int t = idx / row_chunks, r = idx - t * row_chunks;
-    tile[idx] = __ldg(p.in + (static_cast<long long>(t0 + t) * p.n_groups + g0) * p.wc + r);
+    tile[idx] = __ldg(p.in + static_cast<long long>(t0 + t) * p.in_row_chunks + p.in_off_chunks + static_cast<long long>(g0) * p.wc + r);
   }
   __syncthreads();
   // store: chunk fastest, then time, then group  (global writes contiguous per group)
@@ -45,30 +49,6 @@ __global__ void __launch_bounds__(kTurnThreads) corner_turn_kernel(const TurnPar
     const int g = idx / col_chunks, r = idx - g * col_chunks;
     const int t = r / p.wc, k = r - t * p.wc;
     p.out[(static_cast<long long>(g0 + g) * p.n_time + t0) * p.wc + r] = tile[t * row_chunks + g * p.wc + k];
-  }
-}
-
-// Read-out normalisation ("accumulators are ... divided by the number of times they were
-// updated"): out[k] = vis[k] / count, int32 or float sums -> float.  One pass, 16-byte vectors.
-struct NormParams {
-  const void *vis;
-  float *out;
-  long long n;     // scalars (2 per visibility); a multiple of 4
-  float inv_count;
-  int is_int;
-};
-__global__ void __launch_bounds__(256) normalize_kernel(const NormParams p) {
-  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
-  for (long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; k < p.n / 4; k += stride) {
-    float4 o;
-    if (p.is_int) {
-      const int4 v = reinterpret_cast<const int4 *>(p.vis)[k];
-      o = make_float4(v.x * p.inv_count, v.y * p.inv_count, v.z * p.inv_count, v.w * p.inv_count);
-    } else {
-      const float4 v = reinterpret_cast<const float4 *>(p.vis)[k];
-      o = make_float4(v.x * p.inv_count, v.y * p.inv_count, v.z * p.inv_count, v.w * p.inv_count);
-    }
-    reinterpret_cast<float4 *>(p.out)[k] = o;
   }
 }
 

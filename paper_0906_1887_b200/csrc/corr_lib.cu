@@ -2,6 +2,9 @@
 // Plans the tile schedule (descendant of the paper's constant-memory pair lookup table,
 // PAPER.md:117), encodes TMA tensor maps, launches the sm_100a kernels.  No CPU compute path.
 #include "../../include/corr.h"
+#ifdef CORR_DIAG
+#include "../../include/corr_diag.h"
+#endif
 
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -18,7 +21,10 @@
 
 #include "corner_turn.cuh"
 #include "fengine.cuh"
+#include "readout.cuh"
+#ifdef CORR_DIAG
 #include "probe_mma.cuh"
+#endif
 #include "xengine_f32.cuh"
 #include "xengine_f32_n64.cuh"
 #include "xengine_i8.cuh"
@@ -60,24 +66,39 @@ EncodeTiledFn encode_tiled_fn() {
 
 struct MapCacheEntry {
   const void *ptr;
-  CUtensorMap map[3];  // box heights 256, 128, 64 time rows
+  corr::I8Maps maps;  // box heights 256, 128, 64 time rows
 };
+
+constexpr int kMaxSmemI8 = 232448;  // sm_100 opt-in maximum of dynamic shared memory per CTA (227 KB)
 
 }  // namespace
 
+// One planned launch of the int8 kernels: schedule + problem (passed by value into the constant bank), grid, shared memory.
+struct I8Plan {
+  corr::I8Params ip;
+  int grid;
+  size_t smem;
+  int n_batch;  // 0: not planned yet
+};
+
 struct corr_handle {
   int n_inputs, n_chan, n_time, dtype;
+  int n_chan_total, chan0;  // channel window (corr_set_chan_window): d_in is [T][n_chan_total][N], this handle owns chan0 .. chan0 + n_chan - 1
   long long n_baselines;
   size_t in_bytes, vis_bytes;
   int n_sms;
   int turn_mode;
   int probe;
   int accumulate;
-  // CI8 plan
-  int pair_mode, grid_i8, use_pairs;
-  size_t smem_i8;
-  corr::I8Params ip;  // schedule + problem, passed by value into the constant bank at each launch
-  void *d_scratch;  // corner-turn output (standalone mode)
+  long long acc_count;      // batches added since corr_set_accumulate(h, 1)
+  // plan options (corr_set_option)
+  int opt_diag_plan, opt_pairs, opt_wide, opt_units, opt_f32_generic, opt_pdl;
+  // CI8 / CI4 plans
+  int pair_mode;
+  I8Plan plan;        // corr_xengine
+  I8Plan plan_batch;  // corr_xengine_batch, planned for the batch size last seen
+  void *d_scratch;    // corner-turn output (standalone mode)
+  void *d_wide_vis;   // one batch's sums on their way into the wide accumulators (corr_accumulate_wide)
   std::vector<MapCacheEntry> maps;
   // CF32 plan
   int2 *d_items_f32;
@@ -91,6 +112,7 @@ struct corr_handle {
 
 struct corr_fstage {
   int n_inputs, n_fft, n_batch, in_dtype;
+  int device;  // the twiddle table lives in this device's constant memory
   size_t in_bytes, out_bytes;
   void *d_raw[2];  // streaming driver: double-buffered raw voltages
   void *d_spec;    // streaming driver: spectra of the integration in flight
@@ -98,16 +120,18 @@ struct corr_fstage {
 
 namespace {
 
-// Schedule planning (host side of the uniform decode in xengine_i8.cuh).
-void plan_i8(corr_handle *h) {
-  corr::I8Params &ip = h->ip;
+// Schedule planning (host side of the uniform decode in xengine_i8.cuh) for a launch over n_batch integrations.
+void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
+  corr::I8Params &ip = out->ip;
   memset(&ip, 0, sizeof ip);
+  out->n_batch = n_batch;
   const int N = h->n_inputs, C = h->n_chan, T = h->n_time;
-  h->pair_mode = (N == 32) ? 1 : 0;
   const int panels_per_chan = h->pair_mode ? 1 : (2 * N + 127) / 128;
   ip.n_time = T; ip.n_inputs = N; ip.n_chan = C; ip.pair_mode = h->pair_mode;
   ip.n_baselines = h->n_baselines;
+  ip.n_batch = n_batch;
   ip.diag = panels_per_chan == 1;
+  const bool use_pairs = h->dtype == CORR_CI8 && h->opt_pairs && n_batch == 1;  // the 4-bit path and batched launches are single-CTA only
   int max_load = 1;
   if (ip.diag) {
     ip.n_panels = h->pair_mode ? (C + 1) / 2 : C;
@@ -120,36 +144,46 @@ void plan_i8(corr_handle *h) {
     int best_g = 4, best_s = 1;
     double best_t = 1e30;
     const bool small = h->in_bytes <= (64u << 20);
-    for (int g = 4; g >= (small ? 1 : 4); g >>= 1) {
-      const int base = (ip.n_panels + g - 1) / g;
-      int cand_s = 1;
-      double cand_eff = 0.0;
-      for (int s = 1; s <= 64; ++s) {
-        int len = ((T + s - 1) / s + 63) / 64 * 64;
-        if (len < 128 && s > 1) break;
-        const int s_eff = (T + len - 1) / len;
-        if (s_eff != s) continue;
-        const long long n = 1LL * base * s;
+    if (n_batch > 1) {
+      // batched launch: whole integrations (no zeroing nodes), the panel-group width that keeps the SMs evenly
+      // loaded; narrower HBM runs fetch slower (measured relative rates)
+      const double rate[5] = {0.0, 0.70, 0.92, 0.0, 1.0};
+      for (int g = 4; g >= 1; g >>= 1) {
+        const long long n = 1LL * ((ip.n_panels + g - 1) / g) * n_batch;
         const long long rounds = (n + G - 1) / G;
-        // load of the busiest CTA in units of samples vs the mean
-        const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
-        if (small) {
-          // modelled time: rounds x (item bytes at ~80 GB/s per SM) + the fixed cost of a sliced launch
-          const double t = 1e-9 * rounds * (1.0 * g * 128 * std::min(len, T)) / 80.0 + (s > 1 ? 4e-6 : 0.0);
-          if (t < best_t - 1e-7) { best_t = t; best_g = g; best_s = s; }
-        } else {
-          if (eff > cand_eff + 0.02) { cand_eff = eff; cand_s = s; }
-          if (cand_eff >= 0.95) break;
+        const double t = rounds * g / rate[g];
+        if (t < best_t * 0.999) { best_t = t; best_g = g; }
+      }
+    } else {
+      for (int g = 4; g >= (small ? 1 : 4); g >>= 1) {
+        const int base = (ip.n_panels + g - 1) / g;
+        int cand_s = 1;
+        double cand_eff = 0.0;
+        for (int s = 1; s <= 64; ++s) {
+          int len = ((T + s - 1) / s + 63) / 64 * 64;
+          if (len < 128 && s > 1) break;
+          const int s_eff = (T + len - 1) / len;
+          if (s_eff != s) continue;
+          const long long n = 1LL * base * s;
+          const long long rounds = (n + G - 1) / G;
+          // load of the busiest CTA in units of samples vs the mean
+          const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
+          if (small) {
+            // modelled time: rounds x (item bytes at ~80 GB/s per SM) + the fixed cost of a sliced launch
+            const double t = 1e-9 * rounds * (1.0 * g * 128 * std::min(len, T)) / 80.0 + (s > 1 ? 4e-6 : 0.0);
+            if (t < best_t - 1e-7) { best_t = t; best_g = g; best_s = s; }
+          } else {
+            if (eff > cand_eff + 0.02) { cand_eff = eff; cand_s = s; }
+            if (cand_eff >= 0.95) break;
+          }
         }
+        if (!small) best_s = cand_s;
       }
-      if (!small) best_s = cand_s;
     }
-    if (const char *ov = getenv("CORR_DIAG_PLAN")) {  // tests / experiments: "gsize,slices"
-      int g = 0, sl = 0;
-      if (sscanf(ov, "%d,%d", &g, &sl) == 2 && (g == 1 || g == 2 || g == 4) && sl >= 1 && sl <= 64) {
-        const int len = ((T + sl - 1) / sl + 63) / 64 * 64;
-        if (sl == 1 || (len >= 128 && (T + len - 1) / len == sl)) { best_g = g; best_s = sl; }
-      }
+    if (h->opt_diag_plan) {  // corr_set_option(CORR_OPT_DIAG_PLAN): 256 * gsize + slices
+      const int g = h->opt_diag_plan >> 8, sl = h->opt_diag_plan & 255;
+      const int len = ((T + sl - 1) / sl + 63) / 64 * 64;
+      if (sl == 1 || (len >= 128 && (T + len - 1) / len == sl)) { best_g = g; best_s = sl; }
     }
     ip.gsize = best_g;
     ip.n_groups = (ip.n_panels + best_g - 1) / best_g;
@@ -164,8 +198,8 @@ void plan_i8(corr_handle *h) {
     // CTA pairs (cta_group::2) from N_I = 512 up; already from N_I = 256 when the integration is long
     // enough (T >= 2048) for 512-wide tiles, whose epilogue cannot overlap the next tile's MMAs
     const bool long_ok = T >= 2048 && panels_per_chan >= 4;
-    const bool wide_ok = long_ok && !getenv("CORR_NO_WIDE");
-    if (h->use_pairs && (panels_per_chan >= 8 || long_ok)) {
+    const bool wide_ok = long_ok && h->opt_wide;
+    if (use_pairs && (panels_per_chan >= 8 || long_ok)) {
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;
       max_load = 2;
@@ -190,26 +224,26 @@ void plan_i8(corr_handle *h) {
     ip.n_slices = 1;
     ip.slice_len = T;
   }
-  ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices;
+  ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices * n_batch;
   ip.rot = ip.n_kinds > 1 ? 1 : 0;
-  // 32 KB stages: 1 x 256, 2 x 128 or 4 x 64 time rows of 128 B; 48 KB when items fetch 3 panels (3 x 128)
-  ip.stage_bytes = (!ip.diag && max_load == 3) ? 3 * 128 * 128 : 4 * 64 * 128;
+  // 32 KB stages: 1 x 256, 2 x 128 or 4 x 64 time rows of 128 B; 48 KB when items fetch 3 panels (3 x 128).  The 4-bit
+  // mode also keeps the packed bytes of every stage (half as many again): 24 KB stages (3 x 64 rows) there, so that the
+  // ring stays 5 deep instead of 2
+  ip.stage_bytes = (!ip.diag && max_load == 3) ? (h->dtype == CORR_CI4 ? 3 * 64 * 128 : 3 * 128 * 128) : 4 * 64 * 128;
   const int epi_bytes = corr::kEpiWarps * corr::kEpiWarpBytes;  // epilogue staging behind the stage ring
   const int bar_bytes = 512;  // 4 * kMaxStages + 4 mbarriers and the TMEM base address
   const int ring_bytes = h->dtype == CORR_CI4 ? ip.stage_bytes * 3 / 2 : ip.stage_bytes;  // + packed (raw) ring
-  ip.stages = std::min<int>(corr::kMaxStages, (232448 - bar_bytes - epi_bytes) / ring_bytes);
-  h->smem_i8 = static_cast<size_t>(ring_bytes) * ip.stages + epi_bytes + bar_bytes;
+  ip.stages = std::min<int>(corr::kMaxStages, (kMaxSmemI8 - bar_bytes - epi_bytes) / ring_bytes);
+  out->smem = static_cast<size_t>(ring_bytes) * ip.stages + epi_bytes + bar_bytes;
   ip.units = std::min(ip.n_items, ip.pair2 ? h->n_sms / 2 : h->n_sms);
-  if (const char *ue = getenv("CORR_UNITS")) {  // experiments: fewer, fatter CTAs
-    const int u = atoi(ue);
-    if (u >= 1 && !ip.pair2) ip.units = std::min(ip.units, u);
-  }
-  h->grid_i8 = ip.pair2 ? 2 * ip.units : ip.units;
+  if (h->opt_units > 0 && !ip.pair2) ip.units = std::min(ip.units, h->opt_units);  // experiments: fewer, fatter CTAs
+  out->grid = ip.pair2 ? 2 * ip.units : ip.units;
   const int deltas[2] = {ip.units + ip.rot, ip.rot};
   for (int w = 0; w < 2; ++w) { ip.dq[w] = deltas[w] / ip.n_kinds; ip.dr[w] = deltas[w] % ip.n_kinds; }
 }
 
 void plan_f32(corr_handle *h, std::vector<int2> &items) {
+  items.clear();
   const int blocks = (h->n_inputs + corr::kF32Block - 1) / corr::kF32Block;
   for (int c = 0; c < h->n_chan; ++c)
     for (int I = 0; I < blocks; ++I)
@@ -218,7 +252,7 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
   // N_I = 64: (8-channel group, time slice) units; as many slices as fill the SMs evenly (cost = rounds x rows per
   // slice, plus 32 rows for the zeroing node and the reduce-adds of a sliced plan)
   h->n64_groups = h->n64_slices = h->n64_slice_len = 0;
-  if (h->n_inputs == 64 && !getenv("CORR_F32_GENERIC")) {
+  if (h->n_inputs == 64 && !h->opt_f32_generic) {
     const int T = h->n_time, G = h->n_sms;
     h->n64_groups = (h->n_chan + corr::kN64Chan - 1) / corr::kN64Chan;
     long long best = -1;
@@ -240,11 +274,14 @@ int encode_map(corr_handle *h, const void *base, bool turned, int box_rows, CUte
   const cuuint64_t row = static_cast<cuuint64_t>(packed ? 1 : 2) * h->n_inputs;  // bytes per (t, c)
   CUresult r;
   if (!turned) {
+    // the handle's channel window of d_in[T][n_chan_total][N]: x runs over the window only (anything past it is
+    // out of bounds = zero fill), the time stride is the FULL row, the base is moved to the window's first channel
+    const void *win = static_cast<const char *>(base) + static_cast<size_t>(h->chan0) * row;
     cuuint64_t dims[2] = {row * h->n_chan, static_cast<cuuint64_t>(h->n_time)};
-    cuuint64_t strides[1] = {row * h->n_chan};
+    cuuint64_t strides[1] = {row * h->n_chan_total};
     cuuint32_t box[2] = {packed ? 64u : 128u, static_cast<cuuint32_t>(box_rows)};
     cuuint32_t es[2] = {1, 1};
-    r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), dims, strides, box, es,
+    r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(win), dims, strides, box, es,
             CU_TENSOR_MAP_INTERLEAVE_NONE, packed ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   } else {
@@ -262,21 +299,43 @@ int encode_map(corr_handle *h, const void *base, bool turned, int box_rows, CUte
   return CORR_OK;
 }
 
-int get_map(corr_handle *h, const void *base, bool turned, const CUtensorMap **out) {
+int get_map(corr_handle *h, const void *base, bool turned, const corr::I8Maps **out) {
   for (const MapCacheEntry &e : h->maps)
-    if (e.ptr == base) { *out = e.map; return CORR_OK; }
-  if (h->maps.size() >= 64) h->maps.erase(h->maps.begin());
+    if (e.ptr == base) { *out = &e.maps; return CORR_OK; }
+  if (h->maps.size() >= 2 * corr::kMaxBatch) h->maps.erase(h->maps.begin());
   MapCacheEntry e;
   e.ptr = base;
   const int rows[3] = {256, 128, 64};
   for (int m = 0; m < 3; ++m) {
-    int rc = encode_map(h, base, turned, rows[m], &e.map[m]);
+    int rc = encode_map(h, base, turned, rows[m], &e.maps.m[m]);
     if (rc != CORR_OK) return rc;
   }
   h->maps.push_back(e);
-  *out = h->maps.back().map;
+  *out = &h->maps.back().maps;
   return CORR_OK;
 }
+
+// (Re)plans the handle from its shape, window and options; frees / rebuilds the float work-item table.
+int replan(corr_handle *h) {
+  h->maps.clear();
+  h->plan_batch.n_batch = 0;
+  if (h->dtype != CORR_CF32) {
+    h->pair_mode = (h->n_inputs == 32) ? 1 : 0;
+    plan_i8(h, 1, &h->plan);
+    return CORR_OK;
+  }
+  std::vector<int2> items;
+  plan_f32(h, items);
+  cudaFree(h->d_items_f32);
+  h->d_items_f32 = nullptr;
+  cudaError_t e = cudaMalloc(&h->d_items_f32, items.size() * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMemcpy(h->d_items_f32, items.data(), items.size() * sizeof(int2), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess)
+    return fail(e == cudaErrorMemoryAllocation ? CORR_EALLOC : CORR_ECUDA, "corr: work-item table: %s", cudaGetErrorString(e));
+  return CORR_OK;
+}
+
+size_t sample_bytes(int dtype) { return dtype == CORR_CI8 ? 2 : dtype == CORR_CI4 ? 1 : 8; }
 
 }  // namespace
 
@@ -302,7 +361,8 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
     return nullptr;
   }
   if (dtype != CORR_CF32 && n_time > 65535) {
-    fail(CORR_EUNSUPPORTED, "corr_create: CI8 needs n_time <= 65535 so that int32 cannot overflow (got %d)", n_time);
+    fail(CORR_EUNSUPPORTED, "corr_create: %s needs n_time <= 65535 so that int32 cannot overflow (got %d)",
+         dtype == CORR_CI4 ? "CORR_CI4" : "CORR_CI8", n_time);
     return nullptr;
   }
   if (static_cast<unsigned long long>(n_chan) * n_inputs * 2ull >= (1ull << 31)) {
@@ -328,37 +388,40 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->n_chan = n_chan;
   h->n_time = n_time;
   h->dtype = dtype;
+  h->n_chan_total = n_chan;
+  h->chan0 = 0;
   h->n_baselines = static_cast<long long>(n_inputs) * (n_inputs + 1) / 2;
-  h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * (dtype == CORR_CI8 ? 2 : dtype == CORR_CI4 ? 1 : 8);
+  h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * sample_bytes(dtype);
   h->vis_bytes = static_cast<size_t>(n_chan) * h->n_baselines * 8;
   h->n_sms = prop.multiProcessorCount;
   h->turn_mode = CORR_TURN_FUSED;
   h->probe = 0;
   h->accumulate = 0;
+  h->acc_count = 0;
+  h->opt_diag_plan = 0; h->opt_pairs = 1; h->opt_wide = 1; h->opt_units = 0; h->opt_f32_generic = 0; h->opt_pdl = 1;
   h->d_items_f32 = nullptr;
   h->d_scratch = nullptr;
+  h->d_wide_vis = nullptr;
   h->d_stream_in[0] = h->d_stream_in[1] = nullptr;
   h->s_copy = h->s_compute = nullptr;
 
+  // The dynamic shared-memory cap is an attribute of the FUNCTION, not of a handle: it is raised once to the
+  // device maximum so that handles with different footprints can be alive (and launched) side by side.
   cudaError_t e = cudaSuccess;
   if (dtype != CORR_CF32) {
-    h->use_pairs = (dtype == CORR_CI4 || getenv("CORR_NO_PAIRS")) ? 0 : 1;  // the 4-bit path is single-CTA only  // CTA pairs (cta_group::2) for N_I >= 128
-    plan_i8(h);
-    e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(corr::xengine_i4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(corr::xengine_i8_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_i8);
+    e = cudaFuncSetAttribute(corr::xengine_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemI8);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::xengine_i8_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemI8);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::xengine_i4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemI8);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::xengine_i8_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemI8);
   } else {
-    std::vector<int2> items;
-    plan_f32(h, items);
-    e = cudaMalloc(&h->d_items_f32, items.size() * sizeof(int2));
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_items_f32, items.data(), items.size() * sizeof(int2), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && h->n64_groups > 0)
-      e = cudaFuncSetAttribute(corr::xengine_f32_n64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::kN64Smem);
+    e = cudaFuncSetAttribute(corr::xengine_f32_n64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::kN64Smem);
   }
   if (e != cudaSuccess) {
-    fail(e == cudaErrorMemoryAllocation ? CORR_EALLOC : CORR_ECUDA, "corr_create: %s", cudaGetErrorString(e));
+    fail(CORR_ECUDA, "corr_create: %s", cudaGetErrorString(e));
+    corr_destroy(h);
+    return nullptr;
+  }
+  if (replan(h) != CORR_OK) {
     corr_destroy(h);
     return nullptr;
   }
@@ -369,6 +432,7 @@ int corr_destroy(corr_handle *h) {
   if (!h) return CORR_OK;
   cudaFree(h->d_items_f32);
   cudaFree(h->d_scratch);
+  cudaFree(h->d_wide_vis);
   cudaFree(h->d_stream_in[0]);
   cudaFree(h->d_stream_in[1]);
   if (h->s_copy) cudaStreamDestroy(h->s_copy);
@@ -379,11 +443,53 @@ int corr_destroy(corr_handle *h) {
 
 size_t corr_in_bytes(const corr_handle *h) { return h ? h->in_bytes : 0; }
 size_t corr_vis_bytes(const corr_handle *h) { return h ? h->vis_bytes : 0; }
+size_t corr_acc_bytes(const corr_handle *h) { return h ? 2 * h->vis_bytes : 0; }
 int corr_launches_per_call(const corr_handle *h) {
   if (!h) return 0;
   return (h->dtype == CORR_CI8 && h->turn_mode == CORR_TURN_STANDALONE) ? 2 : 1;  // kernels; a memset node precedes them when the integration is time-sliced
 }
 
+int corr_set_option(corr_handle *h, int key, int value) {
+  if (!h) return fail(CORR_EINVAL, "corr_set_option: NULL handle");
+  switch (key) {
+    case CORR_OPT_DIAG_PLAN: {
+      const int g = value >> 8, sl = value & 255;
+      if (value != 0 && !((g == 1 || g == 2 || g == 4) && sl >= 1 && sl <= 64))
+        return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_DIAG_PLAN wants 256 * gsize (1, 2, 4) + slices (1..64), got %d", value);
+      h->opt_diag_plan = value;
+      break;
+    }
+    case CORR_OPT_PAIRS: h->opt_pairs = value ? 1 : 0; break;
+    case CORR_OPT_WIDE: h->opt_wide = value ? 1 : 0; break;
+    case CORR_OPT_UNITS:
+      if (value < 0) return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_UNITS must be >= 0");
+      h->opt_units = value;
+      break;
+    case CORR_OPT_F32_GENERIC: h->opt_f32_generic = value ? 1 : 0; break;
+    case CORR_OPT_PDL: h->opt_pdl = value ? 1 : 0; break;
+    default: return fail(CORR_EINVAL, "corr_set_option: unknown key %d", key);
+  }
+  return replan(h);
+}
+
+int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0) {
+  if (!h) return fail(CORR_EINVAL, "corr_set_chan_window: NULL handle");
+  if (chan0 < 0 || n_chan_total < 1 || static_cast<long long>(chan0) + h->n_chan > n_chan_total)
+    return fail(CORR_EINVAL, "corr_set_chan_window: window %d..%d does not fit %d channels", chan0, chan0 + h->n_chan - 1, n_chan_total);
+  if (static_cast<unsigned long long>(n_chan_total) * h->n_inputs * 2ull >= (1ull << 31))
+    return fail(CORR_EUNSUPPORTED, "corr_set_chan_window: n_chan_total * n_inputs too large");
+  h->n_chan_total = n_chan_total;
+  h->chan0 = chan0;
+  h->in_bytes = static_cast<size_t>(h->n_time) * n_chan_total * h->n_inputs * sample_bytes(h->dtype);
+  h->maps.clear();  // the tensor maps carry the window
+  for (int b = 0; b < 2; ++b) {  // streaming buffers are sized for the full buffer
+    cudaFree(h->d_stream_in[b]);
+    h->d_stream_in[b] = nullptr;
+  }
+  return CORR_OK;
+}
+
+#ifdef CORR_DIAG
 int corr_probe_mma(int m, int n, int mn_major, int iters, double *out) {
   const int fill = mn_major >> 1;  // bit 1 of mn_major: pseudo-random operand bytes; bits 2,3: A == B, wide smem walk
   mn_major &= 1;
@@ -424,32 +530,111 @@ int corr_probe_mma(int m, int n, int mn_major, int iters, double *out) {
   return CORR_OK;
 }
 
+int corr_probe_ffma(int packed, int iters, double *out) {
+  if (iters < 16 || !out) return fail(CORR_EINVAL, "corr_probe_ffma: bad argument");
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = 2 * sms, threads = 512;
+  unsigned long long *d_cyc = nullptr;
+  float *d_sink = nullptr;
+  CUDA_TRY(cudaMalloc(&d_cyc, 2 * blocks * sizeof(unsigned long long)));
+  if (cudaMalloc(&d_sink, static_cast<size_t>(blocks) * threads * sizeof(float)) != cudaSuccess) {
+    cudaFree(d_cyc);
+    return fail(CORR_EALLOC, "corr_probe_ffma: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  corr::ProbeFfmaParams pp{iters, packed ? 1 : 0, 0.999999f, 1e-7f, d_sink, d_cyc};
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  corr::probe_ffma_kernel<<<blocks, threads>>>(pp);  // warm-up
+  cudaEventRecord(e0);
+  corr::probe_ffma_kernel<<<blocks, threads>>>(pp);
+  cudaEventRecord(e1);
+  cudaError_t e = cudaDeviceSynchronize();
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  std::vector<unsigned long long> cyc(2 * blocks);
+  cudaMemcpy(cyc.data(), d_cyc, 2 * blocks * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+  cudaFree(d_cyc);
+  cudaFree(d_sink);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (e != cudaSuccess) return fail(CORR_ECUDA, "corr_probe_ffma: %s", cudaGetErrorString(e));
+  double mean = 0, ns = 0;
+  for (int b = 0; b < blocks; ++b) { mean += static_cast<double>(cyc[2 * b]); ns += static_cast<double>(cyc[2 * b + 1]); }
+  mean /= blocks;
+  ns /= blocks;
+  out[0] = ms;
+  out[1] = 2.0 * 16.0 * iters * static_cast<double>(blocks) * threads / (ns * 1e-9) / 1e12;
+  out[2] = mean / ns * 1e3;
+  return CORR_OK;
+}
+
 int corr_set_probe(corr_handle *h, int mode) {
   if (!h) return fail(CORR_EINVAL, "corr_set_probe: NULL handle");
   h->probe = mode;
   return CORR_OK;
 }
+#endif  // CORR_DIAG
 
 int corr_set_accumulate(corr_handle *h, int on) {
   if (!h) return fail(CORR_EINVAL, "corr_set_accumulate: NULL handle");
   h->accumulate = on ? 1 : 0;
+  h->acc_count = 0;
+  return CORR_OK;
+}
+long long corr_accumulate_count(const corr_handle *h) { return h ? h->acc_count : 0; }
+
+static int launch_normalize(corr_handle *h, const void *d_sums, double count, void *d_out, void *stream, int kind, const char *who) {
+  if (!h || !d_sums || !d_out) return fail(CORR_EINVAL, "%s: NULL argument", who);
+  if (!(count > 0)) return fail(CORR_EINVAL, "%s: count must be positive", who);
+  if ((reinterpret_cast<uintptr_t>(d_sums) | reinterpret_cast<uintptr_t>(d_out)) & 15)
+    return fail(CORR_EINVAL, "%s: pointers must be 16-byte aligned", who);
+  corr::NormParams np;
+  np.vis = d_sums;
+  np.out = static_cast<float *>(d_out);
+  np.n = static_cast<long long>(h->vis_bytes / 4);
+  np.inv_count = static_cast<float>(1.0 / count);
+  np.inv_count_d = 1.0 / count;
+  np.kind = kind;
+  if (np.n % 4) return fail(CORR_EUNSUPPORTED, "%s: odd number of visibilities", who);
+  const int blocks = static_cast<int>(std::min<long long>((np.n / 4 + 255) / 256, static_cast<long long>(h->n_sms) * 8));
+  corr::normalize_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(np);
+  CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }
 
 int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out, void *stream) {
-  if (!h || !d_vis || !d_out) return fail(CORR_EINVAL, "corr_normalize: NULL argument");
-  if (!(count > 0)) return fail(CORR_EINVAL, "corr_normalize: count must be positive");
-  if ((reinterpret_cast<uintptr_t>(d_vis) | reinterpret_cast<uintptr_t>(d_out)) & 15)
-    return fail(CORR_EINVAL, "corr_normalize: pointers must be 16-byte aligned");
-  corr::NormParams np;
-  np.vis = d_vis;
-  np.out = static_cast<float *>(d_out);
-  np.n = static_cast<long long>(h->vis_bytes / 4);
-  np.inv_count = static_cast<float>(1.0 / count);
-  np.is_int = h->dtype != CORR_CF32;
-  if (np.n % 4) return fail(CORR_EUNSUPPORTED, "corr_normalize: odd number of visibilities");
-  const int blocks = static_cast<int>(std::min<long long>((np.n / 4 + 255) / 256, 148 * 8));
-  corr::normalize_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(np);
+  return launch_normalize(h, d_vis, count, d_out, stream, (h && h->dtype == CORR_CF32) ? corr::kSumF32 : corr::kSumI32, "corr_normalize");
+}
+
+int corr_normalize_wide(corr_handle *h, const void *d_acc, double count, void *d_out, void *stream) {
+  if (d_acc && d_acc == d_out) return fail(CORR_EINVAL, "corr_normalize_wide: d_acc and d_out alias");
+  return launch_normalize(h, d_acc, count, d_out, stream, (h && h->dtype == CORR_CF32) ? corr::kSumF64 : corr::kSumI64, "corr_normalize_wide");
+}
+
+int corr_accumulate_wide(corr_handle *h, const void *d_in, void *d_acc, void *stream) {
+  if (!h || !d_in || !d_acc) return fail(CORR_EINVAL, "corr_accumulate_wide: NULL argument");
+  if (reinterpret_cast<uintptr_t>(d_acc) & 15) return fail(CORR_EINVAL, "corr_accumulate_wide: d_acc must be 16-byte aligned");
+  if (!h->d_wide_vis) {
+    cudaError_t e = cudaMalloc(&h->d_wide_vis, h->vis_bytes);
+    if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_accumulate_wide: batch buffer of %zu bytes: %s", h->vis_bytes, cudaGetErrorString(e));
+  }
+  // the batch itself is an ordinary overwriting integration (int32 / float sums of T samples cannot overflow)
+  const int acc_mode = h->accumulate;
+  h->accumulate = 0;
+  const int rc = corr_xengine(h, d_in, h->d_wide_vis, stream);
+  h->accumulate = acc_mode;
+  if (rc != CORR_OK) return rc;
+  corr::FoldParams fp;
+  fp.vis = h->d_wide_vis;
+  fp.acc = d_acc;
+  fp.n = static_cast<long long>(h->vis_bytes / 4);
+  fp.is_int = h->dtype != CORR_CF32;
+  if (fp.n % 4) return fail(CORR_EUNSUPPORTED, "corr_accumulate_wide: odd number of visibilities");
+  const int blocks = static_cast<int>(std::min<long long>((fp.n / 4 + 255) / 256, static_cast<long long>(h->n_sms) * 8));
+  corr::fold_wide_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(fp);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }
@@ -462,11 +647,13 @@ int corr_set_turn(corr_handle *h, int mode) {
     if (h->pair_mode && (h->n_chan & 1))
       return fail(CORR_EUNSUPPORTED, "corr_set_turn: standalone turn with n_inputs == 32 needs an even n_chan");
     if (!h->d_scratch) {
-      cudaError_t e = cudaMalloc(&h->d_scratch, h->in_bytes);
-      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_set_turn: scratch of %zu bytes: %s", h->in_bytes, cudaGetErrorString(e));
+      const size_t bytes = static_cast<size_t>(h->n_time) * h->n_chan * h->n_inputs * 2;
+      cudaError_t e = cudaMalloc(&h->d_scratch, bytes);
+      if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_set_turn: scratch of %zu bytes: %s", bytes, cudaGetErrorString(e));
     }
   }
   h->turn_mode = mode;
+  h->maps.clear();
   return CORR_OK;
 }
 
@@ -480,12 +667,16 @@ static int launch_turn(corr_handle *h, const void *d_in, void *d_out, cudaStream
   tp.n_time = h->n_time;
   tp.n_groups = pair ? h->n_chan / 2 : h->n_chan;
   tp.wc = static_cast<int>(wg / 16);
+  tp.in_row_chunks = static_cast<long long>(h->n_chan_total) * static_cast<long long>(w / 16);
+  tp.in_off_chunks = static_cast<long long>(h->chan0) * static_cast<long long>(w / 16);
   const int max_rows = static_cast<int>(corr::kTurnTileBytes / wg);  // (t, g) rows per tile
   if (max_rows < 1) return fail(CORR_EUNSUPPORTED, "corr_corner_turn: row of %zu bytes exceeds the tile", wg);
   tp.tt = std::min(std::min(32, max_rows), h->n_time);
   tp.gg = std::max(1, std::min(max_rows / tp.tt, tp.n_groups));
-  dim3 grid((tp.n_groups + tp.gg - 1) / tp.gg, (tp.n_time + tp.tt - 1) / tp.tt);
-  corr::corner_turn_kernel<<<grid, corr::kTurnThreads, 0, st>>>(tp);
+  tp.g_tiles = (tp.n_groups + tp.gg - 1) / tp.gg;
+  const long long tiles = static_cast<long long>(tp.g_tiles) * ((tp.n_time + tp.tt - 1) / tp.tt);
+  if (tiles > 0x7fffffffLL) return fail(CORR_EUNSUPPORTED, "corr_corner_turn: %lld tiles exceed the grid limit", tiles);
+  corr::corner_turn_kernel<<<static_cast<unsigned>(tiles), corr::kTurnThreads, 0, st>>>(tp);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }
@@ -501,12 +692,25 @@ int corr_corner_turn(corr_handle *h, const void *d_in, void *d_out, void *stream
   return launch_turn(h, d_in, d_out, static_cast<cudaStream_t>(stream));
 }
 
+// accumulate mode on int32 accumulators: refuse the batch that could overflow them for some input (reading R6)
+static int accumulate_guard(corr_handle *h, long long batches) {
+  if (!h->accumulate || h->dtype == CORR_CF32) return CORR_OK;
+  const long long per_sample = h->dtype == CORR_CI4 ? 2LL * 8 * 8 : 2LL * 128 * 128;
+  if ((h->acc_count + batches) * h->n_time * per_sample >= (1LL << 31))
+    return fail(CORR_EUNSUPPORTED,
+                "corr_xengine: accumulate mode: batch %lld of T = %d samples could overflow the int32 accumulators "
+                "(count * T * %lld >= 2^31); read out and restart, or use corr_accumulate_wide",
+                h->acc_count + batches, h->n_time, per_sample);
+  return CORR_OK;
+}
+
 int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   if (!h) return fail(CORR_EINVAL, "corr_xengine: NULL handle");
   if (!d_in || !d_vis) return fail(CORR_EINVAL, "corr_xengine: NULL device pointer");
   if ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_vis)) & 15)
     return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis must be 16-byte aligned");
   if (d_in == d_vis) return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis alias");
+  if (int rc = accumulate_guard(h, 1)) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (h->dtype == CORR_CF32) {
     if (h->n64_groups > 0) {
@@ -514,11 +718,13 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
       np.in = static_cast<const float2 *>(d_in);
       np.vis = static_cast<float2 *>(d_vis);
       np.n_time = h->n_time; np.n_chan = h->n_chan;
+      np.n_chan_total = h->n_chan_total; np.chan0 = h->chan0;
       np.n_groups = h->n64_groups; np.n_slices = h->n64_slices; np.slice_len = h->n64_slice_len;
       np.add = (h->n64_slices > 1 || h->accumulate) ? 1 : 0;
       if (h->n64_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));
       corr::xengine_f32_n64_kernel<<<h->n64_groups * h->n64_slices, corr::kN64Threads, corr::kN64Smem, st>>>(np);
       CUDA_TRY(cudaGetLastError());
+      if (h->accumulate) ++h->acc_count;
       return CORR_OK;
     }
     corr::F32Params fp;
@@ -529,10 +735,13 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     fp.n_time = h->n_time;
     fp.n_chan = h->n_chan;
     fp.n_inputs = h->n_inputs;
+    fp.n_chan_total = h->n_chan_total;
+    fp.chan0 = h->chan0;
     fp.n_baselines = h->n_baselines;
     fp.accumulate = h->accumulate;
     corr::xengine_f32_kernel<<<h->n_items_f32, h->f32_threads, 0, st>>>(fp);
     CUDA_TRY(cudaGetLastError());
+    if (h->accumulate) ++h->acc_count;
     return CORR_OK;
   }
   const bool turned = h->turn_mode == CORR_TURN_STANDALONE;
@@ -542,38 +751,85 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     if (rc != CORR_OK) return rc;
     src = h->d_scratch;
   }
-  const CUtensorMap *map = nullptr;
-  int rc = get_map(h, src, turned, &map);
+  const corr::I8Maps *maps = nullptr;
+  int rc = get_map(h, src, turned, &maps);
   if (rc != CORR_OK) return rc;
-  corr::I8Params ip = h->ip;
+  corr::I8Params ip = h->plan.ip;
+  const int grid = h->plan.grid;
+  const size_t smem = h->plan.smem;
   ip.turned = turned ? 1 : 0;
   ip.vis = static_cast<int2 *>(d_vis);
   ip.probe = h->probe;
   ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
   ip.accumulate = h->accumulate;
   if (ip.n_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
-  if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<h->grid_i8, corr::kI4Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
-  else if (ip.pair2) corr::xengine_i8_pair_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+  if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<grid, corr::kI4Threads, smem, st>>>(*maps, ip);
+  else if (ip.pair2) corr::xengine_i8_pair_kernel<<<grid, corr::kI8Threads, smem, st>>>(*maps, ip);
   else {
     // programmatic dependent launch: the kernel may start while the preceding kernel of the stream drains (it waits with
     // griddepcontrol.wait before its first global-memory access); worth ~1 us per call on launch-bound inputs (c1: 7.5 ->
     // 6.2 us in a replayed graph).  Only while the stream is being captured into a CUDA graph: launched call by call
     // the attribute costs more host time per launch than it saves on the device.
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cap = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
-    if (cap == cudaStreamCaptureStatusActive && !getenv("CORR_NO_PDL")) {
+    if (h->opt_pdl && cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cap = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
+    if (h->opt_pdl && cap == cudaStreamCaptureStatusActive) {
       cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3(h->grid_i8); cfg.blockDim = dim3(corr::kI8Threads); cfg.dynamicSmemBytes = h->smem_i8; cfg.stream = st;
+      cfg.gridDim = dim3(grid); cfg.blockDim = dim3(corr::kI8Threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
       cudaLaunchAttribute attr[1];
       attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
       attr[0].val.programmaticStreamSerializationAllowed = 1;
       cfg.attrs = attr; cfg.numAttrs = 1;
-      CUDA_TRY(cudaLaunchKernelEx(&cfg, corr::xengine_i8_kernel, map[0], map[1], map[2], ip));
+      CUDA_TRY(cudaLaunchKernelEx(&cfg, corr::xengine_i8_kernel, *maps, ip));
     } else {
-      corr::xengine_i8_kernel<<<h->grid_i8, corr::kI8Threads, h->smem_i8, st>>>(map[0], map[1], map[2], ip);
+      corr::xengine_i8_kernel<<<grid, corr::kI8Threads, smem, st>>>(*maps, ip);
     }
   }
   CUDA_TRY(cudaGetLastError());
+  if (h->accumulate) ++h->acc_count;
+  return CORR_OK;
+}
+
+int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_vis, int n, void *stream) {
+  if (!h) return fail(CORR_EINVAL, "corr_xengine_batch: NULL handle");
+  if (!d_in || !d_vis || n < 1) return fail(CORR_EINVAL, "corr_xengine_batch: NULL pointer array or n < 1");
+  for (int k = 0; k < n; ++k) {
+    if (!d_in[k] || !d_vis[k]) return fail(CORR_EINVAL, "corr_xengine_batch: NULL device pointer at index %d", k);
+    if ((reinterpret_cast<uintptr_t>(d_in[k]) | reinterpret_cast<uintptr_t>(d_vis[k])) & 15)
+      return fail(CORR_EINVAL, "corr_xengine_batch: d_in[%d] and d_vis[%d] must be 16-byte aligned", k, k);
+    if (d_in[k] == d_vis[k]) return fail(CORR_EINVAL, "corr_xengine_batch: d_in[%d] and d_vis[%d] alias", k, k);
+  }
+  // single-launch path: CI8 on single CTAs, fused corner turn, overwrite semantics; everything else = n ordinary calls
+  const bool one_launch = h->dtype == CORR_CI8 && !h->plan.ip.pair2 && h->turn_mode == CORR_TURN_FUSED && !h->accumulate && n > 1;
+  if (!one_launch) {
+    for (int k = 0; k < n; ++k)
+      if (int rc = corr_xengine(h, d_in[k], d_vis[k], stream)) return rc;
+    return CORR_OK;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  for (int k0 = 0; k0 < n; k0 += corr::kMaxBatch) {
+    const int nb = std::min(corr::kMaxBatch, n - k0);
+    if (nb == 1) {
+      if (int rc = corr_xengine(h, d_in[k0], d_vis[k0], stream)) return rc;
+      continue;
+    }
+    if (h->plan_batch.n_batch != nb) plan_i8(h, nb, &h->plan_batch);
+    corr::I8Params ip = h->plan_batch.ip;
+    static thread_local corr::I8Batch bt;  // 25 KB of kernel parameters, copied at launch
+    for (int k = 0; k < nb; ++k) {
+      const corr::I8Maps *maps = nullptr;
+      if (int rc = get_map(h, d_in[k0 + k], false, &maps)) return rc;
+      for (int m = 0; m < 3; ++m) bt.m[k][m] = maps->m[m];
+      bt.vis[k] = static_cast<int2 *>(d_vis[k0 + k]);
+      if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis[k0 + k], 0, h->vis_bytes, st));
+    }
+    ip.turned = 0;
+    ip.vis = nullptr;
+    ip.probe = 0;
+    ip.out_shift = 0;
+    ip.accumulate = 0;
+    corr::xengine_i8_batch_kernel<<<h->plan_batch.grid, corr::kI8Threads, h->plan_batch.smem, st>>>(bt, ip);
+    CUDA_TRY(cudaGetLastError());
+  }
   return CORR_OK;
 }
 
@@ -611,8 +867,13 @@ static int stream_run_impl(corr_handle *h, corr_fstage *f, const void *const *h_
     if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_stream_run_fx: spectra buffer of %zu bytes: %s", f->out_bytes, cudaGetErrorString(e));
   }
   const int n = n_integrations;
-  std::vector<cudaEvent_t> ev(4 * n);  // per integration: copy start, copy end, kernel start, kernel end
-  for (cudaEvent_t &e : ev) CUDA_TRY(cudaEventCreate(&e));
+  std::vector<cudaEvent_t> ev(4 * n, nullptr);  // per integration: copy start, copy end, kernel start, kernel end
+  for (cudaEvent_t &e : ev)
+    if (cudaEventCreate(&e) != cudaSuccess) {
+      for (cudaEvent_t &d : ev)
+        if (d) cudaEventDestroy(d);
+      return fail(CORR_ECUDA, "corr_stream_run: cudaEventCreate: %s", cudaGetErrorString(cudaGetLastError()));
+    }
   int rc = CORR_OK;
   const auto w0 = std::chrono::steady_clock::now();
   for (int k = 0; k < n && rc == CORR_OK; ++k) {
@@ -701,6 +962,7 @@ corr_fstage *corr_fstage_create(int n_inputs, int n_fft, int n_batch) {
   corr_fstage *f = new (std::nothrow) corr_fstage();
   if (!f) { fail(CORR_EALLOC, "corr_fstage_create: out of host memory"); return nullptr; }
   f->n_inputs = n_inputs; f->n_fft = n_fft; f->n_batch = n_batch; f->in_dtype = CORR_CI8;
+  f->device = dev;
   f->d_raw[0] = f->d_raw[1] = f->d_spec = nullptr;
   f->in_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 2;
   f->out_bytes = static_cast<size_t>(n_batch) * n_fft * n_inputs * 8;
@@ -711,6 +973,9 @@ int corr_fstage_run(corr_fstage *f, const void *d_raw, void *d_spec, void *strea
   if (!f || !d_raw || !d_spec) return fail(CORR_EINVAL, "corr_fstage_run: NULL argument");
   if ((reinterpret_cast<uintptr_t>(d_raw) & 15) || (reinterpret_cast<uintptr_t>(d_spec) & 15))
     return fail(CORR_EINVAL, "corr_fstage_run: pointers must be 16-byte aligned");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != f->device)
+    return fail(CORR_EINVAL, "corr_fstage_run: the handle was created on device %d, the current device is %d", f->device, dev);
   corr::FftParams p;
   p.raw = static_cast<const int8_t *>(d_raw);
   p.spec = static_cast<float2 *>(d_spec);

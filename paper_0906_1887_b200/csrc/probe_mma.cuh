@@ -1,4 +1,5 @@
-// probe_mma.cuh -- tcgen05.mma.kind::i8 issue-rate probe (the int8 tensor peak is
+// probe_mma.cuh -- DIAGNOSTICS (built only with -DCORR_DIAG into libcorr_diag.so; include/corr_diag.h):
+// tcgen05.mma.kind::i8 issue-rate probe (the int8 tensor peak is
 // not in MEASURED_PEAKS.json, so it is measured here).  One CTA per SM; one thread issues `iters`
 // back-to-back MMAs on zero-filled shared-memory operands (values do not matter for timing) into
 // two alternating TMEM accumulators, then commits and waits.  No global traffic at all.
@@ -69,6 +70,51 @@ __global__ void __launch_bounds__(128, 1) probe_mma_kernel(const ProbeParams p) 
     tc_fence_after();
     tmem_dealloc(tmem_base, 512);
   }
+}
+
+// FP32 FMA issue-rate probe (the "alu" roofline denominator of the float X-engine): every thread runs `iters`
+// rounds of 16 independent register-resident FMAs -- scalar FFMA (packed = 0) or packed fma.rn.f32x2 (packed = 1,
+// the instruction xengine_f32_n64_kernel uses).  No memory traffic inside the loop.
+struct ProbeFfmaParams {
+  int iters, packed;
+  float b, c;                  // runtime multiplier / addend (keeps the chain from being folded)
+  float *sink;                 // [gridDim.x * blockDim.x]
+  unsigned long long *cycles;  // [2 * gridDim.x]: SM cycles, globaltimer ns of the loop (thread 0 of each CTA)
+};
+__global__ void __launch_bounds__(512, 2) probe_ffma_kernel(const ProbeFfmaParams p) {
+  float2 a[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) a[k] = make_float2(threadIdx.x * 1e-3f + k, blockIdx.x * 1e-3f - k);
+  const float2 b2 = make_float2(p.b, p.b), c2 = make_float2(p.c, p.c);
+  unsigned long long g0 = 0, g1 = 0;
+  if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+  const long long t0 = clock64();
+  if (p.packed) {
+    for (int it = 0; it < p.iters; ++it) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(reinterpret_cast<unsigned long long &>(a[k]))
+                     : "l"(reinterpret_cast<const unsigned long long &>(b2)), "l"(reinterpret_cast<const unsigned long long &>(c2)));
+    }
+  } else {
+    for (int it = 0; it < p.iters; ++it) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(a[k].x) : "f"(p.b), "f"(p.c));
+        asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(a[k].y) : "f"(p.b), "f"(p.c));
+      }
+    }
+  }
+  const long long t1 = clock64();
+  if (threadIdx.x == 0) {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+    p.cycles[2 * blockIdx.x] = static_cast<unsigned long long>(t1 - t0);
+    p.cycles[2 * blockIdx.x + 1] = g1 - g0;
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += a[k].x + a[k].y;
+  p.sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
 }  // namespace corr

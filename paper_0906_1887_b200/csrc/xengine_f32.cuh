@@ -26,6 +26,7 @@ struct F32Params {
   const int2 *items;  // {chan, I | J << 16}
   int n_items;
   int n_time, n_chan, n_inputs;
+  int n_chan_total, chan0;  // d_in is [T][n_chan_total][N]; this handle correlates channels chan0 .. chan0 + n_chan - 1
   long long n_baselines;
   int accumulate;  // 1: d_vis += this integration; every element has exactly one writer
 };
@@ -76,9 +77,9 @@ __global__ void __launch_bounds__(kF32Threads) xengine_f32_kernel(const F32Param
     active = true;
   }
 
-  const long long row_stride = static_cast<long long>(p.n_chan) * p.n_inputs;
-  const long long col_i = static_cast<long long>(chan) * p.n_inputs + I * kF32Block;
-  const long long col_j = static_cast<long long>(chan) * p.n_inputs + J * kF32Block;
+  const long long row_stride = static_cast<long long>(p.n_chan_total) * p.n_inputs;
+  const long long col_i = static_cast<long long>(p.chan0 + chan) * p.n_inputs + I * kF32Block;
+  const long long col_j = static_cast<long long>(p.chan0 + chan) * p.n_inputs + J * kF32Block;
 
   const int nvc_i = min(32, (p.n_inputs - I * kF32Block) / 2);
   const int nvc_j = min(32, (p.n_inputs - J * kF32Block) / 2);

@@ -4,9 +4,9 @@
 // Why a second kernel: in xengine_f32.cuh (4 x 4 tiles) the shared-memory RETURN path is as busy as the FMA pipe --
 // an LDS.128 returns 512 B per warp = 4 cycles of the SM's 128 B/cycle whatever the broadcast, and a 4 x 4 tile needs
 // 4 of them per 64 FFMA.  An 8 x 4 tile needs 6 per 128 FFMA (0.75 load cycles per FMA cycle).  The 64-input lower
-// triangle is 72 such tiles; 8 ADJACENT channels share a CTA so that 576 threads = 18 full warps are all busy
-// (4 KB contiguous per time row in d_in), and the integration is cut into time slices so that the (group, slice)
-// units fill the 148 SMs evenly (c5: 192 groups x 3 slices = 576 units = 3.9 per SM); slices add their partial sums
+// triangle is 72 such tiles; 7 ADJACENT channels share a CTA so that 504 threads = 16 warps (4 per scheduler, 128
+// registers each) are all busy (3.5 KB contiguous per time row in d_in), and the integration is cut into time slices
+// so that the (group, slice) units fill the 148 SMs evenly (c5: 220 groups x 2 slices = 440 units = 2.97 per SM); slices add their partial sums
 // with red.global.add.v2.f32 into a zeroed d_vis (FP32 sums in a different order: within the 1e-5 tolerance, reading R8).
 //
 // V_ij = sum_t x_i conj(x_j), FP32 FMA accumulation; no tensor cores (TF32 cannot meet 1e-5).
@@ -20,16 +20,17 @@ namespace corr {
 
 constexpr int kN64Chan = 7;                    // channels per CTA
 constexpr int kN64Tiles = 72;                  // 8 x 4 tiles of the 64-input lower triangle
-constexpr int kN64Threads = kN64Chan * kN64Tiles;  // 576
+constexpr int kN64Threads = kN64Chan * kN64Tiles;  // 504
 constexpr int kN64TB = 16;                     // time rows per stage
 constexpr int kN64Stages = 3;
-constexpr int kN64RowF4 = kN64Chan * 32;       // float4 per time row of a group (4 KB)
-constexpr int kN64Smem = kN64Stages * kN64TB * kN64RowF4 * 16;  // 96 KB
+constexpr int kN64RowF4 = kN64Chan * 32;       // float4 per time row of a group (3.5 KB)
+constexpr int kN64Smem = kN64Stages * kN64TB * kN64RowF4 * 16;  // 168 KB
 
 struct F32N64Params {
   const float2 *in;  // [T][C][64]
   float2 *vis;       // [C][2080]
   int n_time, n_chan, n_groups, n_slices, slice_len;
+  int n_chan_total, chan0;  // d_in is [T][n_chan_total][64]; this handle correlates channels chan0 .. chan0 + n_chan - 1
   int add;           // 1: reduce-add into d_vis (time slices or accumulate mode); 0: plain stores
 };
 
@@ -63,8 +64,8 @@ __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F
   const int sw = (tj >> 2) & 1;
   const bool active = cg < n_chan_here;
 
-  const long long row_f4 = static_cast<long long>(p.n_chan) * 32;  // float4 per time row of d_in
-  const float4 *src0 = reinterpret_cast<const float4 *>(p.in) + static_cast<long long>(c0) * 32;
+  const long long row_f4 = static_cast<long long>(p.n_chan_total) * 32;  // float4 per time row of d_in
+  const float4 *src0 = reinterpret_cast<const float4 *>(p.in) + static_cast<long long>(p.chan0 + c0) * 32;
   const int valid_f4 = n_chan_here * 32;
 
   auto load_stage = [&](int s) {

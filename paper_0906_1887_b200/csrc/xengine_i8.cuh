@@ -16,7 +16,8 @@
 // touches stays in uniform registers, which is what lets one thread issue at the tensor-pipe rate.
 //
 // Warp roles (384 threads, 1 CTA/SM, persistent):
-//   warp 8   TMA producer: box {128 B along the chan*input axis, bk time rows}, SWIZZLE_128B.
+//   warps 8, 11  TMA producers (one thread each, alternate stages): box {128 B along the chan*input
+//            axis, bk time rows}, SWIZZLE_128B.
 //            This strided box load IS the corner turn: it lands as the
 //            canonical MN-major operand tile, so the input is read from HBM exactly once.
 //   warp 9   MMA issuer (one thread): tcgen05.mma.kind::i8, M=128, N=128|256, K=32.
@@ -39,6 +40,7 @@ constexpr int kPanelBytes = 128;  // bytes of the chan*input axis per panel = 64
 constexpr int kAccCols = 256;     // TMEM columns per accumulator ring entry (two 128-column blocks)
 constexpr int kMaxStages = 8;
 constexpr int kMaxKinds = 1056;   // slab kinds per channel at N_I = 4096 (64 panels, column pairs)
+constexpr int kMaxBatch = 64;     // integrations per launch of the batched entry point (corr_xengine_batch)
 
 struct I8Params {
   // ---- schedule (uniform) ----
@@ -46,8 +48,9 @@ struct I8Params {
   int gsize;         // diag: adjacent panels per item (4, or 2 / 1 for small problems)
   int n_kinds;       // items per group (diag: 1)
   int n_slices;      // time slices per integration (> 1 => results are accumulated with red.add)
-  int slice_len;     // samples per slice (multiple of 256 when n_slices > 1)
-  int n_items;       // n_groups * n_kinds * n_slices
+  int slice_len;     // samples per slice (multiple of 64 when n_slices > 1)
+  int n_batch;       // integrations per launch (1 except for xengine_i8_batch_kernel)
+  int n_items;       // n_groups * n_kinds * n_slices * n_batch
   int rot;           // per-round rotation of the CTA -> item map (spreads the kinds over the CTAs)
   int dq[2], dr[2];  // (grid + rot) and rot, each split as quotient / remainder by n_kinds (host-computed)
   int diag;          // item kind
@@ -81,21 +84,31 @@ struct I8Item {
   int chan, I, J0;   // slab: channel, row panel, first column panel; diag: first panel in J0
 };
 
-// Position of a CTA in the schedule: item g = (s * n_groups + grp) * n_kinds + k, walked WITHOUT
+// Tensor maps of one input buffer (box heights 256 / 128 / 64 time rows) and the per-integration arguments of a
+// batched launch: one launch walks a schedule that spans n_batch integrations (the paper's remedy for small
+// transfers: "process large batches of data per call"; 32 blocks per call).
+struct I8Maps { CUtensorMap m[3]; };
+struct I8Batch {
+  CUtensorMap m[kMaxBatch][3];
+  int2 *vis[kMaxBatch];
+};
+
+// Position of a CTA in the schedule: item g = ((bi * n_slices + s) * n_groups + grp) * n_kinds + k, walked WITHOUT
 // divisions (additions, compares and constant-bank reads only), so that ptxas keeps the whole walk
 // and everything decoded from it in uniform registers.  Round r of CTA b takes item
 // r * grid + (b + r * rot) mod grid.
 struct I8Iter {
-  int s, grp, k, b;
+  int bi, s, grp, k, b;
 };
 __device__ __forceinline__ void iter_carry(const I8Params &p, I8Iter &c) {
   if (c.k >= p.n_kinds) { c.k -= p.n_kinds; ++c.grp; }
   while (c.grp >= p.n_groups) { c.grp -= p.n_groups; ++c.s; }
+  while (c.s >= p.n_slices && c.bi < p.n_batch) { c.s -= p.n_slices; ++c.bi; }
 }
 __device__ __forceinline__ I8Iter iter_init(const I8Params &p) {
   I8Iter c;
   c.b = static_cast<int>(blockIdx.x) >> p.pair2;
-  c.s = 0; c.grp = 0; c.k = c.b;
+  c.bi = 0; c.s = 0; c.grp = 0; c.k = c.b;
   while (c.k >= p.n_kinds) { c.k -= p.n_kinds; ++c.grp; }
   iter_carry(p, c);
   return c;
@@ -108,7 +121,7 @@ __device__ __forceinline__ void iter_next(const I8Params &p, I8Iter &c) {
   c.grp += p.dq[w];
   iter_carry(p, c);
 }
-__device__ __forceinline__ bool iter_valid(const I8Params &p, const I8Iter &c) { return c.s < p.n_slices; }
+__device__ __forceinline__ bool iter_valid(const I8Params &p, const I8Iter &c) { return c.bi < p.n_batch; }
 
 // Decode of a schedule position (all inputs are kernel parameters / uniform counters).
 __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c, int rank = 0) {

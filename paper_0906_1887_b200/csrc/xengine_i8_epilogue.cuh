@@ -22,8 +22,8 @@ constexpr int kEpiWarpBytes = 16 * kEpiRowBytes;  // 4224 B per epilogue warp
 // kAtomic: reduce-add into d_vis (time-sliced or accumulating items) instead of plain stores.  kShift: 8 for
 // 4-bit input (operands are 16 x the samples), else 0.  Both are compile-time so that the plain-store path is
 // the bare minimum per value: one SHFL, one IMAD (v + sgn * partner), one conflict-free STS.
-template <bool kAtomic, int kShift>
-__device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_base, uint8_t *stage_buf,
+template <bool kAtomic, int kShift, bool kBatch>
+__device__ __forceinline__ void i8_epilogue(const I8Params &p, int2 *const *vis_list, uint32_t tmem_base, uint8_t *stage_buf,
                                             uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
                                             int hsel, int lane, int rank, bool pair, int probe) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
@@ -39,6 +39,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
   for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
     if (!iter_valid(p, cur)) continue;
     const I8Item it = decode_item(p, cur, rank);
+    int2 *const vis = kBatch ? vis_list[cur.bi] : p.vis;  // output of this item's integration
     const int n_chunks = (it.nblk + 1) >> 1;
     for (int q = 0; q < n_chunks; ++q) {
       const uint32_t e = ring + q;
@@ -110,7 +111,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
                 const long long e0 = static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j0;
                 const int sh = static_cast<int>(e0 & 1);
                 const int2 *srow = reinterpret_cast<const int2 *>(stage_buf + lane * kRowB) + sh;  // element 0
-                int2 *grow = p.vis + e0;
+                int2 *grow = vis + e0;
                 int head = sh;                         // one leading element if e0 is odd
                 int body = (cnt - head) & ~1;          // aligned pairs
                 if (cnt < head) { head = cnt; body = 0; }
@@ -136,7 +137,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, uint32_t tmem_bas
             // of 32, so every row and column of the half block exists; only diagonal blocks need the j <= i test.
             const int j = j0 + lane;
             const int i = i0_w;
-            int2 *row = p.vis + (static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j);
+            int2 *row = vis + (static_cast<long long>(chan_w) * p.n_baselines + i * (i + 1) / 2 + j);
             const int2 *src = reinterpret_cast<const int2 *>(stage_buf) + lane;
             int2 val[16];
 #pragma unroll

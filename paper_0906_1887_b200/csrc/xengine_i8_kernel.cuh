@@ -28,9 +28,10 @@ __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_
   }
 }
 
-template <bool kPair, bool kProbe, bool kPacked = false>
-__device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, const CUtensorMap &tmap128,
-                                                const CUtensorMap &tmap64, const I8Params &p) {
+// maps: the tensor maps of the input(s), [n_batch][3] (box heights 256 / 128 / 64 time rows); vis_list: the output of
+// every integration of a batched launch (kBatch), else unused (p.vis).
+template <bool kPair, bool kProbe, bool kPacked = false, bool kBatch = false>
+__device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *const *vis_list, const I8Params &p) {
   // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
   // 128-byte swizzle needs: [stage ring][epilogue staging][mbarriers + TMEM base].
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -49,8 +50,8 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
 
   // programmatic dependent launch (single-CTA kernels): the next call's launch, barrier set-up and TMEM allocation may
   // overlap this call's tail; every role that touches global memory waits for the preceding grid first
-  if (!kPair) griddep_launch_dependents();
-  const int probe = kProbe ? p.probe : 0;  // diagnostics compile away in the production instantiation
+  if (!kPair && !kBatch) griddep_launch_dependents();
+  const int probe = kProbe ? p.probe : 0;  // diagnostics (-DCORR_DIAG builds only) compile away in the product
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const int n_rounds = (p.n_items + p.units - 1) / p.units;
@@ -60,9 +61,9 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
   // roles sit in the HIGHEST warps because the SMSP arbiter favours higher warp ids: they are the critical
   // path and must not queue behind eight busy epilogue warps.
   if (warp == kProducerWarp && lane == 0) {
-    tma_prefetch_desc(&tmap256);
-    tma_prefetch_desc(&tmap128);
-    tma_prefetch_desc(&tmap64);
+    tma_prefetch_desc(&maps[0]);
+    tma_prefetch_desc(&maps[1]);
+    tma_prefetch_desc(&maps[2]);
     for (int s = 0; s < p.stages; ++s) {
       mbar_init(&full_bar[s], kPacked ? kExpandWarps : 1);  // packed: the expand warps publish the int8 stage
       mbar_init(&empty_bar[s], 1);
@@ -90,7 +91,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     const int pw = (warp == kProducerWarp) ? 0 : 1;
     int iter = 0;
     if (elect_one() && !(probe & 8)) {
-      if (!kPair) griddep_wait();  // d_in may have been written by the preceding kernel of the stream
+      if (!kPair && !kBatch) griddep_wait();  // d_in may have been written by the preceding kernel of the stream
       const uint64_t pol = policy_evict_normal();
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
@@ -99,7 +100,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
         const I8Item it = decode_item(p, cur, rank);
-        const CUtensorMap *map = it.map == 0 ? &tmap256 : (it.map == 1 ? &tmap128 : &tmap64);
+        const CUtensorMap *map = maps + (kBatch ? 3 * cur.bi : 0) + it.map;
         const uint32_t panel_bytes = static_cast<uint32_t>(it.bk) * kPanelBytes;
         for (int t = it.t0; t < it.t1; t += it.bk, ++iter) {
           if ((iter & 1) != pw) {
@@ -270,16 +271,16 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
     }
   } else if (warp < kEpiWarps && !(probe & 4)) {
     // ===================================================================== epilogue
-    if (!kPair) griddep_wait();  // d_vis may still be written (or read) by the preceding kernel of the stream
+    if (!kPair && !kBatch) griddep_wait();  // d_vis may still be written (or read) by the preceding kernel of the stream
     const int ew = warp & 3;         // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
     constexpr int kShift = kPacked ? 8 : 0;
     if (p.n_slices > 1 || p.accumulate)
-      i8_epilogue<true, kShift>(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
-                                acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+      i8_epilogue<true, kShift, kBatch>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                        acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
     else
-      i8_epilogue<false, kShift>(p, tmem_base, epi_stage + warp * kEpiWarpBytes,
-                             acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+      i8_epilogue<false, kShift, kBatch>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                         acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 
   tc_fence_before();
@@ -291,25 +292,34 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap &tmap256, cons
 }
 
 __global__ void __launch_bounds__(kI8Threads, 1)
-xengine_i8_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
-                  const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  if (p.probe) xengine_i8_body<false, true>(tmap256, tmap128, tmap64, p);
-  else         xengine_i8_body<false, false>(tmap256, tmap128, tmap64, p);
+xengine_i8_kernel(const __grid_constant__ I8Maps tm, const __grid_constant__ I8Params p) {
+#ifdef CORR_DIAG
+  if (p.probe) { xengine_i8_body<false, true>(tm.m, nullptr, p); return; }
+#endif
+  xengine_i8_body<false, false>(tm.m, nullptr, p);
 }
 
-// 4-bit packed input (the paper's "1-byte mode"): 16 warps, the last four expand nibbles to int8.
+// One launch over n_batch integrations (corr_xengine_batch; "process large batches of data per call",
+// 32 blocks of spectra per GPU call): the schedule walk carries the integration index, which selects
+// the tensor maps and the output of the item.  All SMs stay busy on inputs too small to fill the chip alone (c1).
+__global__ void __launch_bounds__(kI8Threads, 1)
+xengine_i8_batch_kernel(const __grid_constant__ I8Batch bt, const __grid_constant__ I8Params p) {
+  xengine_i8_body<false, false, false, true>(&bt.m[0][0], bt.vis, p);
+}
+
+// 4-bit packed input (the paper's "1-byte mode"): 20 warps, the last eight expand nibbles to int8.
 __global__ void __launch_bounds__(kI4Threads, 1)
-xengine_i4_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
-                  const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  xengine_i8_body<false, false, true>(tmap256, tmap128, tmap64, p);
+xengine_i4_kernel(const __grid_constant__ I8Maps tm, const __grid_constant__ I8Params p) {
+  xengine_i8_body<false, false, true>(tm.m, nullptr, p);
 }
 
 // CTA pairs: tcgen05.mma.cta_group::2, M = 256 (one 128-row panel per CTA), each CTA stages half of B.
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kI8Threads, 1)
-xengine_i8_pair_kernel(const __grid_constant__ CUtensorMap tmap256, const __grid_constant__ CUtensorMap tmap128,
-                       const __grid_constant__ CUtensorMap tmap64, const __grid_constant__ I8Params p) {
-  if (p.probe) xengine_i8_body<true, true>(tmap256, tmap128, tmap64, p);
-  else         xengine_i8_body<true, false>(tmap256, tmap128, tmap64, p);
+xengine_i8_pair_kernel(const __grid_constant__ I8Maps tm, const __grid_constant__ I8Params p) {
+#ifdef CORR_DIAG
+  if (p.probe) { xengine_i8_body<true, true>(tm.m, nullptr, p); return; }
+#endif
+  xengine_i8_body<true, false>(tm.m, nullptr, p);
 }
 
 }  // namespace corr

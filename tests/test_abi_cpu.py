@@ -16,8 +16,8 @@ needs_nvcc = pytest.mark.skipif(shutil.which("nvcc") is None and not os.path.exi
     os.path.join(ROOT, "paper_0906_1887_b200", "libcorr.so")), reason="no nvcc and no prebuilt libcorr.so")
 
 
-def header_symbols():
-    text = open(os.path.join(ROOT, "include", "corr.h")).read()
+def header_symbols(name="corr.h"):
+    text = open(os.path.join(ROOT, "include", name)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(corr_[a-z0-9_]+)\s*\(", text)))
 
@@ -31,6 +31,33 @@ def test_library_exports_every_declared_symbol():
     for s in syms:
         assert hasattr(L, s), f"{s} declared in include/corr.h but not exported"
     assert set(pkg.EXPORTS) == set(syms)
+    # the diagnostics (include/corr_diag.h) live in libcorr_diag.so only: the product library carries neither the
+    # probe entry points nor the probe-instrumented kernel instantiations
+    diag = header_symbols("corr_diag.h")
+    assert set(pkg.DIAG_EXPORTS) == set(diag) and {"corr_probe_mma", "corr_probe_ffma", "corr_set_probe"} <= set(diag)
+    for s in diag:
+        assert not hasattr(L, s), f"{s} is a diagnostic but libcorr.so exports it"
+    D = pkg.diag_lib()
+    for s in syms + diag:
+        assert hasattr(D, s), f"{s} missing from libcorr_diag.so"
+
+
+@needs_nvcc
+def test_product_library_reads_no_environment_and_has_one_instantiation_per_kernel():
+    """Plan knobs go through corr_set_option, not getenv; each hot kernel is instantiated once in libcorr.so."""
+    import subprocess
+    import paper_0906_1887_b200 as pkg
+    pkg.lib()
+    for f in os.listdir(os.path.join(ROOT, "paper_0906_1887_b200", "csrc")):
+        assert "getenv" not in open(os.path.join(ROOT, "paper_0906_1887_b200", "csrc", f)).read(), f
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump not available")
+    lib = os.path.join(ROOT, "paper_0906_1887_b200", "libcorr.so")
+    out = subprocess.run(["cuobjdump", "-elf", lib], capture_output=True, text=True, timeout=300).stdout
+    names = set(re.findall(r"\.text\.(_ZN4corr\w+)", out))
+    kernels = sorted(n for n in names if "xengine" in n or "fengine" in n)
+    assert len(kernels) == 8, kernels   # i8, i8_batch, i8_pair, i4, f32, f32_n64, fengine, fengine_ci4
+    assert not any("probe" in n for n in names), names
 
 
 @needs_nvcc
@@ -50,6 +77,11 @@ def test_no_cpu_fallback_without_device():
     L = pkg.lib()
     assert L.corr_destroy(None) == pkg.CORR_OK
     assert L.corr_xengine(None, None, None, None) == pkg.CORR_EINVAL
+    assert L.corr_xengine_batch(None, None, None, 1, None) == pkg.CORR_EINVAL
+    assert L.corr_set_option(None, pkg.CORR_OPT_PAIRS, 0) == pkg.CORR_EINVAL
+    assert L.corr_set_chan_window(None, 4, 0) == pkg.CORR_EINVAL
+    assert L.corr_accumulate_wide(None, None, None, None) == pkg.CORR_EINVAL
+    assert L.corr_accumulate_count(None) == 0 and L.corr_acc_bytes(None) == 0
     # F-stage: same rules (no device -> error code; bad shapes rejected before any device work)
     with pytest.raises(pkg.CorrError) as e:
         pkg.corr_fstage_create(64, 128, 10)

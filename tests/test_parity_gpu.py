@@ -28,9 +28,11 @@ def _threads():
     return oracle.host_threads()
 
 
-def run_ci8(pkg, x, turn=None):
+def run_ci8(pkg, x, turn=None, options=()):
     T, C, N, _ = x.shape
     h = pkg.corr_create(N, C, T, "ci8")
+    for key, value in options:
+        h.set_option(key, value)
     if turn is not None:
         h.set_turn(turn)
     d_in = torch.from_numpy(x).cuda()
@@ -43,9 +45,11 @@ def run_ci8(pkg, x, turn=None):
     return out
 
 
-def run_cf32(pkg, x):
+def run_cf32(pkg, x, options=()):
     T, C, N, _ = x.shape
     h = pkg.corr_create(N, C, T, "cf32")
+    for key, value in options:
+        h.set_option(key, value)
     d_in = torch.from_numpy(x).cuda()
     vis = h.empty_vis()
     vis.fill_(float("nan"))
@@ -85,12 +89,18 @@ def test_ci8_uniform_full_range_bit_exact(pkg, N, C, T):
 
 
 @pytest.mark.parametrize("N,C,T", [(512, 2, 100), (256, 2, 2100), (1024, 1, 64)])
-def test_ci8_single_cta_slabs_when_pairs_are_disabled(pkg, N, C, T, monkeypatch):
-    """CORR_NO_PAIRS=1 (the A/B knob of DESIGN.md section 11) selects the single-CTA slab schedule."""
-    monkeypatch.setenv("CORR_NO_PAIRS", "1")
+def test_ci8_single_cta_slabs_when_pairs_are_disabled(pkg, N, C, T):
+    """corr_set_option(CORR_OPT_PAIRS, 0) (the A/B knob of DESIGN.md section 7) selects the single-CTA slab schedule."""
     w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
-    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+    assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_PAIRS, 0)]), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (512, 1, 2081)])
+def test_ci8_pair_tiles_without_the_wide_ones(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_WIDE, 0)]), oracle.xengine_ci8(x, threads=_threads()))
 
 
 def test_ci8_zero_input(pkg):
@@ -219,23 +229,32 @@ def test_mma_probe_runs_at_the_tensor_rate(pkg):
 # default to whole integrations of 1-2 panels; "4,s" is what the large configs (c2) run, incl. the reduce-add path.
 @pytest.mark.parametrize("plan", ["4,1", "4,3", "2,1", "2,2", "1,1", "1,4"])
 @pytest.mark.parametrize("N,C,T", [(64, 11, 700), (32, 13, 530), (64, 1, 129)])
-def test_ci8_diag_plans_bit_exact(pkg, monkeypatch, plan, N, C, T):
-    monkeypatch.setenv("CORR_DIAG_PLAN", plan)
+def test_ci8_diag_plans_bit_exact(pkg, plan, N, C, T):
+    g, sl = (int(v) for v in plan.split(","))
     w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
-    assert np.array_equal(run_ci8(pkg, x), oracle.xengine_ci8(x, threads=_threads()))
+    out = run_ci8(pkg, x, options=[(pkg.CORR_OPT_DIAG_PLAN, 256 * g + sl)])
+    assert np.array_equal(out, oracle.xengine_ci8(x, threads=_threads()))
+
+
+def test_set_option_rejects_bad_arguments(pkg):
+    h = pkg.corr_create(64, 2, 100, "ci8")
+    for key, value in [(99, 1), (pkg.CORR_OPT_DIAG_PLAN, 256 * 3 + 1), (pkg.CORR_OPT_DIAG_PLAN, 256 * 4 + 65), (pkg.CORR_OPT_UNITS, -1)]:
+        with pytest.raises(pkg.CorrError) as e:
+            h.set_option(key, value)
+        assert e.value.status == pkg.CORR_EINVAL
+    pkg.corr_destroy(h)
 
 
 # N_I = 64 float path (xengine_f32_n64_kernel: 7-channel groups, time slices with reduce-add): group tails (C not a
 # multiple of 7), slice tails, one slice (plain stores) and many; and the generic 4 x 4 kernel forced on the same shapes.
 @pytest.mark.parametrize("generic", [False, True])
 @pytest.mark.parametrize("C,T", [(1, 1), (7, 16), (8, 17), (15, 100), (150, 33), (23, 700), (300, 260)])
-def test_cf32_n64_paths_within_tolerance(pkg, monkeypatch, generic, C, T):
-    if generic:
-        monkeypatch.setenv("CORR_F32_GENERIC", "1")
+def test_cf32_n64_paths_within_tolerance(pkg, generic, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c5"], n_inputs=64, n_chan=C, n_time=T)
     x = w.generate()
-    f32_tolerance_check(run_cf32(pkg, x), oracle.xengine_cf32(x, threads=_threads()), 64)
+    out = run_cf32(pkg, x, options=[(pkg.CORR_OPT_F32_GENERIC, 1)] if generic else ())
+    f32_tolerance_check(out, oracle.xengine_cf32(x, threads=_threads()), 64)
 
 
 def test_ci8_cuda_graph_with_dependent_launches(pkg):
