@@ -24,8 +24,9 @@ if ROOT not in sys.path:
 METRIC = "xengine_complex_macs_per_s"
 UNIT = "CMAC/s"
 L2_BYTES = 126 * 1024 * 1024
-# provisional arithmetic peaks: int8 dense = 2 x measured bf16 burst; FP32 FMA = 148 SM x 128 x 2 x f
-FP32_PEAK_FLOPS = 148 * 128 * 2 * 1.965e9
+# FP32 FMA peak: measured live by the library's FFMA issue-rate probe (corr_probe_ffma); this derived figure
+# (148 SMs x 128 lanes x 2 flops x max clock) is printed beside it and used only if the probe cannot run
+FP32_PEAK_DERIVED = 148 * 128 * 2 * 1.965e9
 
 
 def measured_peaks():
@@ -34,6 +35,21 @@ def measured_peaks():
         d = json.load(open(p))
         return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]), "source": "measured"}
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback"}
+
+
+def fp32_peak_flops(peaks, pkg=None):
+    """FP32 FMA peak in FLOP/s: the best of the scalar and packed issue-rate probes, else the derived figure."""
+    if "fp32_flops" not in peaks:
+        peaks["fp32_flops"], peaks["fp32_source"] = FP32_PEAK_DERIVED, "derived: 148 SM x 128 lanes x 2 x 1.965 GHz"
+        if pkg is not None:
+            try:
+                r = {k: max(pkg.probe_ffma(packed=(k == "packed"), iters=8192)["tflops"] for _ in range(3)) for k in ("scalar", "packed")}
+                peaks["fp32_probe"] = r
+                peaks["fp32_flops"] = max(r.values()) * 1e12
+                peaks["fp32_source"] = "measured: corr_probe_ffma (register-resident FMA chains, best of scalar FFMA / packed FFMA2)"
+            except Exception:
+                pass
+    return peaks["fp32_flops"]
 
 
 def int8_peak_tops(peaks, pkg=None):
@@ -54,7 +70,7 @@ def roofline_times(w, peaks):
     """(t_hbm, t_alu) seconds per integration: north_star's lower-of-two roofline."""
     t_a = w.in_bytes / (peaks["hbm_gbs"] * 1e9)
     ops = 8.0 * w.cmacs
-    peak_ops = int8_peak_tops(peaks) * 1e12 if w.dtype == "ci8" else FP32_PEAK_FLOPS
+    peak_ops = int8_peak_tops(peaks) * 1e12 if w.dtype == "ci8" else fp32_peak_flops(peaks)
     return t_a, ops / peak_ops
 
 
@@ -106,11 +122,26 @@ def make_inputs(w, n_buffers, torch, rank=0):
     return [torch.from_numpy(w.generate(integration=k + 1000 * rank)).cuda() for k in range(n_buffers)]
 
 
-def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None):
-    """Device-resident timing of `steps` corr_xengine calls.  Returns dict with per-step seconds."""
-    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, w.dtype)
+def shard_plan(w, world, rank):
+    """Strong scaling: rank `rank` of `world` owns the channel window
+    [c0, c1) of the ONE seeded cube every rank holds; returns (c0, c1, arguments of corr_create for the window,
+    arguments of corr_set_chan_window)."""
+    c0, c1 = shard_channels(w.n_chan, world, rank)
+    return c0, c1, (w.n_inputs, c1 - c0, w.n_time, w.dtype), (w.n_chan, c0)
+
+
+def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None, window=None):
+    """Device-resident timing of `steps` corr_xengine calls.  Returns dict with per-step seconds.  window = (c0, c1):
+    the handle correlates that channel window of the full cube in place (strong scaling)."""
+    if window is None:
+        h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, w.dtype)
+    else:
+        h = pkg.corr_create(w.n_inputs, window[1] - window[0], w.n_time, w.dtype)
+        h.set_chan_window(w.n_chan, window[0])
     n_buf = 1 if w.in_bytes > 2 * L2_BYTES else min(64, -(-3 * L2_BYTES // w.in_bytes))
-    bufs = make_inputs(w, n_buf, torch, rank)
+    if w.in_bytes <= (64 << 20) and w.dtype == "ci8":
+        n_buf = 64  # two batched launches of 32 integrations on distinct buffers
+    bufs = make_inputs(w, n_buf, torch, 0 if window is not None else rank)  # strong scaling: the same cube on every rank
     vis = h.empty_vis()
     stream = torch.cuda.current_stream()
     for k in range(warmup):
@@ -130,7 +161,7 @@ def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None):
     per = sorted(ev[k].elapsed_time(ev[k + 1]) * 1e-3 for k in range(steps))
     out = {"total_s": total, "mean_s": total / steps, "median_s": per[len(per) // 2], "best_s": per[0],
            "launches": steps * h.launches_per_call, "n_buffers": n_buf, "handle": h, "bufs": bufs, "vis": vis}
-    if n_buf > 1 and not sampler:
+    if n_buf > 1 and not sampler and window is None:
         # isolated latency of one call (device idle before and after), SURVEY H3
         lone = []
         for k in range(10):
@@ -194,6 +225,34 @@ def time_config(pkg, torch, w, steps, warmup, rank=0, sampler=None):
             del g
             for hh in hs:
                 hh.destroy()
+            # the batched entry point (corr_xengine_batch): ONE launch per `nb` integrations, ONE
+            # stream; a graph of n_buf / nb launches over the n_buf distinct buffers (> 2 x L2 in total), replayed
+            for nb in (32, 64):
+                if n_buf % nb:
+                    continue
+                vs = [h.empty_vis() for _ in range(nb)]
+                with torch.cuda.stream(side):
+                    h.xengine_batch(bufs[:nb], vs, side)
+                    torch.cuda.synchronize()
+                    g = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g, stream=side):
+                        for c in range(n_buf // nb):
+                            h.xengine_batch(bufs[c * nb:(c + 1) * nb], vs, side)
+                    for _ in range(2):
+                        g.replay()
+                    torch.cuda.synchronize()
+                    reps = []
+                    for _ in range(max(5, -(-steps // n_buf))):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record(side)
+                        g.replay()
+                        e1.record(side)
+                        torch.cuda.synchronize()
+                        reps.append(e0.elapsed_time(e1) * 1e-3 / n_buf)
+                out[f"batch{nb}_s"] = sorted(reps)[len(reps) // 2]
+                if nb == 32:
+                    out["batch_vis"], out["batch_bufs"] = vs, bufs[n_buf - nb:]
+                del g
     return out
 
 
@@ -236,15 +295,25 @@ def cpu_baseline(w, target_s=12.0, gpu_vis=None):
     t0 = time.perf_counter()
     fn(x, 0, 1, threads=1)
     one = max(time.perf_counter() - t0, 1e-4)            # one channel, one thread
+    # (i) the plain single-threaded oracle -- the paper's comparator was single-threaded C -- on the
+    # first k1 channels (about 2 s; work is exactly linear and independent in the channel)
+    k1 = int(min(w.n_chan, max(1, 2.0 / one)))
+    t0 = time.perf_counter()
+    fn(x, 0, k1, threads=1)
+    sec1 = time.perf_counter() - t0
+    # (ii) the same loops under OpenMP over channels on all cores
     k = int(max(cores, min(w.n_chan, target_s * cores / one)))
     k = min(w.n_chan, k)
     t0 = time.perf_counter()
     ref = fn(x, 0, k, threads=cores)
     sec = time.perf_counter() - t0
     out = {"value": w.n_time * k * w.n_baselines / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-           "sample": f"channels 0..{k - 1} of {w.n_chan}, all T={w.n_time} samples, {sec:.1f} s, OpenMP over channels"}
+           "sample": f"channels 0..{k - 1} of {w.n_chan}, all T={w.n_time} samples, {sec:.1f} s, OpenMP over channels",
+           "single_thread": {"value": w.n_time * k1 * w.n_baselines / sec1, "unit": UNIT, "cores": 1,
+                             "sample": f"channels 0..{k1 - 1} of {w.n_chan}, all T={w.n_time} samples, {sec1:.1f} s, one thread"}}
     if gpu_vis is not None:
-        g = gpu_vis[:k]
+        k = min(k, len(gpu_vis))   # a channel-sharded rank holds its window only (rank 0: channels 0 .. c1-1)
+        g, ref = gpu_vis[:k], ref[:k]
         if w.dtype == "ci8":
             out["parity"] = "bit-exact" if np.array_equal(g, ref) else "MISMATCH"
         else:
@@ -255,6 +324,34 @@ def cpu_baseline(w, target_s=12.0, gpu_vis=None):
             worst = float(np.max(err / np.maximum(sc, 1e-300)))
             out["parity"] = f"max err/scale {worst:.2e} (tol 1e-5)" if worst <= 1e-5 else f"OUT OF TOLERANCE {worst:.2e}"
     return out
+
+
+def cpu_baseline_stream_parity(w, ring, d_vis, n_integrations, per_integration=2):
+    """The streamed run of config 5 checked against the float64 oracle: for EACH of the integrations, a few sampled
+    channels at north_star's tolerance |dV| <= 1e-5 sqrt(|V_ii V_jj|) (V_ii, V_jj from the oracle).  `ring` holds
+    the distinct pinned host inputs; integration k streamed ring[k % len(ring)]."""
+    import numpy as np
+    import oracle
+    rng = np.random.default_rng(2024)
+    N = w.n_inputs
+    ii, jj = np.tril_indices(N)
+    worst, checked = 0.0, 0
+    cache = {}
+    for k in range(n_integrations):
+        chans = sorted(int(c) for c in rng.choice(w.n_chan, size=per_integration, replace=False))
+        for c in chans:
+            key = (k % len(ring), c)
+            if key not in cache:
+                cache[key] = oracle.xengine_cf32(ring[key[0]].numpy(), c, c + 1, threads=1)[0]
+            ref = cache[key]
+            g = d_vis[k, c].cpu().numpy().astype(np.float64)
+            sc = np.sqrt(np.abs(ref[ii * (ii + 1) // 2 + ii, 0] * ref[jj * (jj + 1) // 2 + jj, 0]))
+            err = np.hypot(g[:, 0] - ref[:, 0], g[:, 1] - ref[:, 1])
+            worst = max(worst, float(np.max(err / np.maximum(sc, 1e-300))))
+            checked += 1
+    verdict = "within tolerance" if worst <= 1e-5 else "OUT OF TOLERANCE"
+    return {"result": verdict, "max_err_over_scale": worst, "tolerance": 1e-5, "integrations": n_integrations,
+            "channels_checked": checked, "sample": f"{per_integration} seeded random channels of every integration, all 2080 baselines each"}
 
 
 def run_reference(args, w):
@@ -327,6 +424,42 @@ def reduce_max(dist, value, device):
     return float(t.item())
 
 
+def tensor_fracs(w, sec, peaks):
+    """A tensor-bound int8 config against BOTH int8 denominators: the library's issue-rate probe and the guide's rule
+    (another dtype's measured peak x the nominal ratio = 2 x measured bf16 burst)."""
+    ops = 8.0 * w.cmacs
+    return {"frac_probe_peak": ops / (int8_peak_tops(peaks) * 1e12) / sec, "int8_probe_tops": int8_peak_tops(peaks),
+            "frac_2xbf16": ops / (2.0 * peaks["bf16_tflops"] * 1e12) / sec, "int8_2xbf16_tops": 2.0 * peaks["bf16_tflops"]}
+
+
+def corner_turn_entry(pkg, torch, w, h, x, steps=10):
+    """The standalone corner-turn kernel (second realisation) on this config: the kernel alone
+    (reads and writes the input once: 2 x in_bytes of HBM traffic) and corr_xengine routed through it."""
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ev[0].record(stream)
+        for k in range(steps):
+            fn()
+            ev[k + 1].record(stream)
+        torch.cuda.synchronize()
+        per = sorted(ev[k].elapsed_time(ev[k + 1]) * 1e-3 for k in range(steps))
+        return per[len(per) // 2]
+
+    scratch = torch.empty_like(x)
+    vis = h.empty_vis()
+    sec_turn = timed(lambda: h.corner_turn(x, scratch, stream))
+    del scratch
+    h.set_turn(pkg.CORR_TURN_STANDALONE)
+    sec_path = timed(lambda: h.xengine(x, vis, stream))
+    h.set_turn(pkg.CORR_TURN_FUSED)
+    return {"turn_kernel_ms": sec_turn * 1e3, "turn_kernel_gbs": 2.0 * w.in_bytes / sec_turn / 1e9,
+            "xengine_ms_through_standalone_turn": sec_path * 1e3}
+
+
 def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     """Kernel-only numbers of another config (context for 'vs N_I'; not a bench line of its own)."""
     import corrgen
@@ -337,6 +470,15 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     out = {"n_inputs": w.n_inputs, "value": w.cmacs / sec, "unit": UNIT, "ms": sec * 1e3,
            "bound": "hbm" if t_a >= t_b else ("tensor" if w.dtype == "ci8" else "alu"),
            "roofline_ms": max(t_a, t_b) * 1e3, "frac": max(t_a, t_b) / sec, "n_buffers": r["n_buffers"]}
+    if w.dtype == "ci8" and t_b > 0.5 * t_a:   # tensor-bound or at the ridge: both int8 denominators
+        out.update(tensor_fracs(w, sec, peaks))
+        out["frac_2xbf16_roofline"] = max(t_a, 8.0 * w.cmacs / (2.0 * peaks["bf16_tflops"] * 1e12)) / sec
+    if w.dtype == "cf32":
+        out["fp32_peak_tflops"] = fp32_peak_flops(peaks) / 1e12
+        out["fp32_peak_source"] = peaks["fp32_source"]
+        out["kernel"] = "xengine_f32_n64_kernel" if w.n_inputs == 64 else "xengine_f32_kernel"
+    if key in ("c2", "c4"):
+        out["corner_turn"] = corner_turn_entry(pkg, torch, w, r["handle"], r["bufs"][0])
     if "graph_s" in r:
         out["timing"] = f"CUDA graph of {r['n_buffers']} calls on rotating buffers, replayed (steady state)"
         out["ms_eager"] = r["median_s"] * 1e3  # call by call from Python: host launch-bound
@@ -344,19 +486,39 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     if "graph4_s" in r:
         out["ms_4streams"] = r["graph4_s"] * 1e3  # the same calls spread over 4 streams of one graph (they overlap)
         out["frac_4streams"] = max(t_a, t_b) / r["graph4_s"]
+    if "batch32_s" in r:
+        # corr_xengine_batch: one launch per 32 (64) integrations, one stream, distinct buffers
+        out["ms_batched"] = r["batch32_s"] * 1e3
+        out["frac_batched"] = max(t_a, t_b) / r["batch32_s"]
+        out["batched"] = (f"per integration; graph of {r['n_buffers'] // 32} corr_xengine_batch launches x 32 integrations on "
+                          f"{r['n_buffers']} distinct buffers ({r['n_buffers'] * w.in_bytes / 1e6:.0f} MB), replayed")
+        if "batch64_s" in r:
+            out["ms_batched64"] = r["batch64_s"] * 1e3
+            out["frac_batched64"] = max(t_a, t_b) / r["batch64_s"]
+        # the batched outputs equal the single-call outputs of the same inputs (which the GPU tests pin to the oracle)
+        single = r["handle"].empty_vis()
+        same = True
+        for k in (0, 17, 31):
+            r["handle"].xengine(r["batch_bufs"][k], single)
+            same = same and bool(torch.equal(single, r["batch_vis"][k]))
+        out["batched_equals_single_calls"] = same
     if w.dtype == "cf32" and w.n_integrations > 1:
         # streaming driver: n_integrations back-to-back integrations from pinned host buffers,
         # H2D of k+1 under the kernel of k; a ring of 4 distinct pinned buffers stands in for the 20
         ring = [torch.from_numpy(w.generate(integration=k)).pin_memory() for k in range(4)]
         hs = [ring[k % 4] for k in range(w.n_integrations)]
         r["handle"].stream_run(hs)  # warm-up (allocates the two device buffers)
-        _, st = r["handle"].stream_run(hs)
+        d_vis, st = r["handle"].stream_run(hs)
         rate = w.n_integrations * w.n_time * w.n_chan / st["device_s"]       # complex samples/s per input
         out["stream"] = {"integrations": w.n_integrations, "device_s": st["device_s"], "kernel_s": st["kernel_s"],
                          "h2d_s": st["h2d_s"], "h2d_gbs": w.n_integrations * w.in_bytes / st["h2d_s"] / 1e9,
                          "samples_per_s_per_input": rate, "rtf_vs_15.36MSps": rate / 15.36e6,
                          "rtf_vs_paper_1.28MSps": rate / 1.28e6, "e2e_cmacs_per_s": w.n_integrations * w.cmacs / st["device_s"]}
-        del ring, hs
+        try:   # BASELINE.json config 5: the streamed run "checks against a float64 oracle"
+            out["stream"]["parity"] = cpu_baseline_stream_parity(w, ring, d_vis, w.n_integrations)
+        except Exception as e:
+            out["stream"]["parity"] = {"result": "not checked", "error": str(e)[:200]}
+        del ring, hs, d_vis
     r["handle"].destroy()
     del r
     torch.cuda.empty_cache()
@@ -482,17 +644,19 @@ def main():
     pkg.lib()
     peaks = measured_peaks()
     int8_peak_tops(peaks, pkg)
+    fp32_peak_flops(peaks, pkg)
     dev = torch.device("cuda", torch.cuda.current_device())
 
     w_full = w
+    window = None
     if args.scaling == "strong" and world > 1:
-        c0, c1 = shard_channels(w.n_chan, world, rank)
-        w = corrgen.scaled(w, n_chan=c1 - c0, seed=w.seed + 7919 * rank)  # this rank's channel slice (own seeded data)
+        c0, c1, _, _ = shard_plan(w, world, rank)
+        window = (c0, c1)   # this rank's channel window of the ONE cube (same seed on every rank), read in place
     sampler = ClockSampler(index=torch.cuda.current_device()) if rank == 0 else None
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    r = time_config(pkg, torch, w, args.steps, args.warmup, rank, sampler)
+    r = time_config(pkg, torch, w, args.steps, args.warmup, rank, sampler, window)
     if dist is not None:
         dist.barrier()
     total_s = reduce_max(dist, r["total_s"], dev)
@@ -503,7 +667,7 @@ def main():
         torch.cuda.synchronize()
     gpu_vis = r["vis"].cpu().numpy()
 
-    e2e = time_e2e(pkg, torch, w, h, args.e2e_steps, rank)
+    e2e = time_e2e(pkg, torch, w, h, args.e2e_steps, 0 if window is not None else rank)
     e2e_sec = reduce_max(dist, e2e["ms_per_step"] * 1e-3, dev)
     e2e["value"] = (w_full.cmacs if (args.scaling == "strong" and world > 1) else world * w.cmacs) / e2e_sec
     e2e["ms_per_step"] = e2e_sec * 1e3
@@ -517,11 +681,22 @@ def main():
     elif w.dtype == "ci8":
         roof = {"bound": "tensor", "achieved": 8.0 * w.cmacs / kern / 1e12, "peak": int8_peak_tops(peaks), "unit": "TOP/s"}
     else:
-        roof = {"bound": "alu", "achieved": 8.0 * w.cmacs / kern / 1e12, "peak": FP32_PEAK_FLOPS / 1e12, "unit": "TFLOP/s"}
+        roof = {"bound": "alu", "achieved": 8.0 * w.cmacs / kern / 1e12, "peak": fp32_peak_flops(peaks) / 1e12, "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["peak_source"] = peaks["int8_source"] if roof["bound"] == "tensor" else peaks["source"]
+    roof["peak_source"] = peaks["int8_source"] if roof["bound"] == "tensor" else (peaks["fp32_source"] if roof["bound"] == "alu" else peaks["source"])
     roof["int8_peak_tops"] = int8_peak_tops(peaks)
-    roof["kernel"] = "xengine_i8_kernel" if w.dtype == "ci8" else "xengine_f32_kernel"
+    roof["int8_peak_source"] = peaks["int8_source"]
+    roof["fp32_peak_measured"] = fp32_peak_flops(peaks) / 1e12
+    roof["fp32_peak_source"] = peaks["fp32_source"]
+    roof["fp32_peak_derived"] = FP32_PEAK_DERIVED / 1e12
+    if "fp32_probe" in peaks:
+        roof["fp32_probe_tflops"] = peaks["fp32_probe"]
+    if roof["bound"] == "tensor":
+        roof.update(tensor_fracs(w, kern, peaks))
+    if w.dtype != "ci8":
+        roof["kernel"] = "xengine_f32_n64_kernel" if w.n_inputs == 64 else "xengine_f32_kernel"
+    else:
+        roof["kernel"] = "xengine_i8_pair_kernel" if (w.n_inputs >= 512 or (w.n_inputs >= 256 and w.n_time >= 2048)) else "xengine_i8_kernel"
     roof["kernel_ms"] = kern * 1e3
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     traffic = json.load(open(tpath)).get(args.config) if os.path.exists(tpath) else None
@@ -532,7 +707,9 @@ def main():
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak",
             "vs_baseline": None, "dtype": "s8 x s8 -> s32" if w.dtype == "ci8" else "f32", "data": "synthetic",
             "config": {"workload": workload_name(w), "n_inputs": w.n_inputs, "n_chan": w.n_chan, "n_time": w.n_time,
-                       "parallelism": f"channel-independent replicas x{world}" if world > 1 else "single GPU",
+                       "parallelism": (f"channels sharded over {world} GPUs, each reading its window of the one cube in place (corr_set_chan_window)"
+                                       if (world > 1 and args.scaling == "strong") else
+                                       f"channel-independent replicas x{world}" if world > 1 else "single GPU"),
                        "l2": (f"input {w.in_bytes / 1e6:.0f} MB per step > 126 MB L2, no flush needed" if r["n_buffers"] == 1
                               else f"rotating {r['n_buffers']} distinct input buffers ({r['n_buffers'] * w.in_bytes / 1e6:.0f} MB > L2)")},
             "clocks": sampler.summary() if sampler else None,

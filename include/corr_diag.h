@@ -35,9 +35,9 @@ int corr_probe_mma(int m, int n, int mn_major, int iters, double *out);
 
 /*
  * corr_probe_ffma -- FP32 FMA issue rate on the current device (the "alu" roofline denominator of the
- * float X-engine): 2 CTAs x 512 threads per SM, 16 independent register-resident FMA chains per thread,
+ * float X-engine): one CTA of 1024 threads per SM, 16 independent register-resident FMA chains per thread,
  * `iters` rounds; packed = 0: scalar fma.rn.f32, 1: fma.rn.f32x2 (what xengine_f32_n64_kernel issues).
- * out[0] = kernel ms, out[1] = TFLOP/s over all SMs (2 flops per FMA, over the loop itself),
+ * out[0] = kernel ms, out[1] = TFLOP/s over all SMs (2 flops per FMA, over the slowest SM's loop),
  * out[2] = effective SM MHz during the loop.
  */
 int corr_probe_ffma(int packed, int iters, double *out);

@@ -81,7 +81,9 @@ struct ProbeFfmaParams {
   float *sink;                 // [gridDim.x * blockDim.x]
   unsigned long long *cycles;  // [2 * gridDim.x]: SM cycles, globaltimer ns of the loop (thread 0 of each CTA)
 };
-__global__ void __launch_bounds__(512, 2) probe_ffma_kernel(const ProbeFfmaParams p) {
+__global__ void __launch_bounds__(1024, 1) probe_ffma_kernel(const ProbeFfmaParams p) {
+  extern __shared__ uint8_t ffma_pad[];  // 200 KB of dynamic shared memory: exactly one CTA per SM
+  if (p.iters < 0) ffma_pad[threadIdx.x] = 0;
   float2 a[8];
 #pragma unroll
   for (int k = 0; k < 8; ++k) a[k] = make_float2(threadIdx.x * 1e-3f + k, blockIdx.x * 1e-3f - k);

@@ -37,6 +37,20 @@ def test_channel_sharding_covers_every_channel_once():
         assert max(sizes) - min(sizes) <= 1
 
 
+def test_shard_plan_gives_window_arguments():
+    """Strong scaling: every rank's corr_create / corr_set_chan_window arguments tile the ONE cube."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import corrgen
+    w = corrgen.CONFIGS["c2"]
+    covered = []
+    for rank in range(5):
+        c0, c1, create_args, window_args = bench.shard_plan(w, 5, rank)
+        assert create_args == (w.n_inputs, c1 - c0, w.n_time, w.dtype) and window_args == (w.n_chan, c0)
+        covered += list(range(c0, c1))
+    assert covered == list(range(w.n_chan))
+
+
 def test_reference_arm_prints_contract_line():
     env = dict(os.environ, OMP_NUM_THREADS="2")
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "c1",
@@ -57,6 +71,15 @@ rank, world, d = bench.dist_setup(2)
 assert world == 2 and d is not None
 t = bench.reduce_max(d, 1.0 + rank, torch.device("cpu"))
 assert t == 2.0, t
+import corrgen
+w = corrgen.scaled(corrgen.CONFIGS["c2"], n_chan=11)
+c0, c1, create_args, window_args = bench.shard_plan(w, world, rank)
+# the two ranks' windows tile the cube: exchange the edges and check (the only "collective" is this test's own)
+edges = torch.tensor([float(c0), float(c1)])
+gathered = [torch.zeros(2) for _ in range(world)]
+dist.all_gather(gathered, edges)
+assert gathered[0][0] == 0 and gathered[0][1] == gathered[1][0] and gathered[1][1] == w.n_chan, gathered
+assert create_args[1] == c1 - c0 and window_args == (w.n_chan, c0)
 d.barrier()
 d.destroy_process_group()
 print("ok", rank)
