@@ -166,10 +166,13 @@ int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
 enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
                                    panels per work item and `slices` (1..64) time slices; 0 = automatic       */
        CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
-       CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default)                                     */
+       CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
        CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
-       CORR_OPT_PDL = 6         /* 0: never launch programmatically inside a stream capture; 1 (default)      */ };
+       CORR_OPT_PDL = 6,        /* 0: never launch programmatically inside a stream capture; 1 (default)      */
+       CORR_OPT_COLLECT = 7,    /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */
+       CORR_OPT_RESIDENT = 8    /* 0: no resident-A plan (N_I >= 512, T <= 1024: a CTA keeps its A panel of the whole
+                                   integration in shared memory); 1 (default)                                 */ };
 int corr_set_option(corr_handle *h, int key, int value);
 
 /*

@@ -20,9 +20,14 @@ extern "C" {
 /*
  * corr_set_probe -- switches engines of the CI8 kernel off so that the others can be timed alone.  Bit
  * mask: 1 = skip the MMAs, 2 = skip the TMA loads (producer only hand-shakes), 4 = no epilogue, 8 = no
- * producer and no stage hand-shake at all, 16 = epilogue without its global stores; 0 = normal.
+ * producer and no stage hand-shake at all, 16 = epilogue without its global stores, 128 = results stay correct, the
+ * MMA issuer and the first TMA producer of every CTA (pair) count the SM cycles they spend waiting; 0 = normal.
+ * corr_probe_stats (after a launch with bit 128, synchronised by the caller): out[0..3] = mean over the CTAs (pairs)
+ * of the kernel's cycles, the MMA issuer's cycles waiting for a loaded stage, its cycles waiting for a free
+ * TMEM accumulator, and the producer's cycles waiting for a free stage.
  */
 int corr_set_probe(corr_handle *h, int mode);
+int corr_probe_stats(corr_handle *h, double *out);
 
 /*
  * corr_probe_mma -- tcgen05.mma.kind::i8 issue rate on the current device (the int8 tensor peak of the

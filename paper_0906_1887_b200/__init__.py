@@ -15,7 +15,7 @@ from . import build as _build
 CORR_CI8, CORR_CF32, CORR_CI4 = 0, 1, 2
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
 CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
-CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL = 1, 2, 3, 4, 5, 6
+CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL, CORR_OPT_COLLECT, CORR_OPT_RESIDENT = 1, 2, 3, 4, 5, 6, 7, 8
 
 # include/corr.h (the product ABI, libcorr.so)
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
@@ -25,7 +25,7 @@ EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "co
            "corr_set_option",
            "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx", "corr_fstage_set_input")
 # include/corr_diag.h (diagnostics, libcorr_diag.so only)
-DIAG_EXPORTS = ("corr_set_probe", "corr_probe_mma", "corr_probe_ffma")
+DIAG_EXPORTS = ("corr_set_probe", "corr_probe_stats", "corr_probe_mma", "corr_probe_ffma")
 
 _lib = None
 _diag = False
@@ -72,6 +72,7 @@ def _bind(path, diag):
     L.corr_set_option.restype, L.corr_set_option.argtypes = ci, [vp, ci, ci]
     if diag:
         L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
+        L.corr_probe_stats.restype, L.corr_probe_stats.argtypes = ci, [vp, ctypes.POINTER(ctypes.c_double)]
         L.corr_probe_mma.restype = ci
         L.corr_probe_mma.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.corr_probe_ffma.restype = ci
@@ -173,6 +174,13 @@ class Correlator:
         """Diagnostics build only (use_diag_build())."""
         if lib().corr_set_probe(self._h, mode) != CORR_OK:
             _raise()
+
+    def probe_stats(self):
+        """Diagnostics build only: mean cycles per CTA (pair) of the last launch with probe bit 128."""
+        out = (ctypes.c_double * 4)()
+        if lib().corr_probe_stats(self._h, out) != CORR_OK:
+            _raise()
+        return {"cycles": out[0], "mma_wait_loads": out[1], "mma_wait_tmem": out[2], "producer_wait_stage": out[3]}
 
     # -- corr_set_accumulate / corr_normalize
     def set_accumulate(self, on=True):

@@ -92,13 +92,14 @@ struct corr_handle {
   int accumulate;
   long long acc_count;      // batches added since corr_set_accumulate(h, 1)
   // plan options (corr_set_option)
-  int opt_diag_plan, opt_pairs, opt_wide, opt_units, opt_f32_generic, opt_pdl;
+  int opt_diag_plan, opt_pairs, opt_wide, opt_units, opt_f32_generic, opt_pdl, opt_collect, opt_resident;
   // CI8 / CI4 plans
   int pair_mode;
   I8Plan plan;        // corr_xengine
   I8Plan plan_batch;  // corr_xengine_batch, planned for the batch size last seen
   void *d_scratch;    // corner-turn output (standalone mode)
   void *d_wide_vis;   // one batch's sums on their way into the wide accumulators (corr_accumulate_wide)
+  unsigned long long *d_diag_stats;  // diagnostics build only (corr_probe_stats)
   std::vector<MapCacheEntry> maps;
   // CF32 plan
   int2 *d_items_f32;
@@ -201,9 +202,18 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     int k = 0;
     // CTA pairs (cta_group::2) from N_I = 512 up; already from N_I = 256 when the integration is long
     // enough (T >= 2048) for 512-wide tiles, whose epilogue cannot overlap the next tile's MMAs
-    const bool long_ok = T >= 2048 && panels_per_chan >= 4;
+    const bool long_ok = (T >= 2048 || h->opt_wide == 2) && panels_per_chan >= 4;
     const bool wide_ok = long_ok && h->opt_wide;
-    if (use_pairs && (panels_per_chan >= 8 || long_ok)) {
+    if (use_pairs && panels_per_chan >= 8 && !long_ok && T <= 128 * corr::kResMaxSub && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
+      // resident-A plan (xengine_i8_resident.cuh): the A panel of the whole integration stays in shared memory; an item
+      // is a unit of two row pairs (pp - 1 - u and u: pp + 1 tiles in every unit)
+      ip.pair2 = 1;
+      ip.resident = 1;
+      ip.a_sub = (T + 127) / 128;
+      const int pp = (panels_per_chan + 1) / 2;
+      for (int u = 0; u < (pp + 1) / 2; ++u) ip.kinds[k++] = static_cast<unsigned short>(u);
+      max_load = 1;
+    } else if (use_pairs && (panels_per_chan >= 8 || long_ok)) {
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;
       max_load = 2;
@@ -236,9 +246,11 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
   ip.stage_bytes = (!ip.diag && max_load == 3) ? (h->dtype == CORR_CI4 ? 3 * 64 * 128 : 3 * 128 * 128) : 4 * 64 * 128;
   const int epi_bytes = corr::kEpiWarps * corr::kEpiWarpBytes;  // epilogue staging behind the stage ring
   const int bar_bytes = 512;  // 4 * kMaxStages + 4 mbarriers and the TMEM base address
+  if (ip.resident) ip.stage_bytes = corr::kResSubBytes;
+  const int a_bytes = ip.resident ? ip.a_sub * corr::kResSubBytes : 0;
   const int ring_bytes = h->dtype == CORR_CI4 ? ip.stage_bytes * 3 / 2 : ip.stage_bytes;  // + packed (raw) ring
-  ip.stages = std::min<int>(corr::kMaxStages, (kMaxSmemI8 - bar_bytes - epi_bytes) / ring_bytes);
-  out->smem = static_cast<size_t>(ring_bytes) * ip.stages + epi_bytes + bar_bytes;
+  ip.stages = std::min<int>(corr::kMaxStages, (kMaxSmemI8 - bar_bytes - epi_bytes - a_bytes) / ring_bytes);
+  out->smem = static_cast<size_t>(ring_bytes) * ip.stages + a_bytes + epi_bytes + bar_bytes;
   ip.units = std::min(ip.n_items, ip.pair2 ? h->n_sms / 2 : h->n_sms);
   if (h->opt_units > 0 && !ip.pair2) ip.units = std::min(ip.units, h->opt_units);  // experiments: fewer, fatter CTAs
   out->grid = ip.pair2 ? 2 * ip.units : ip.units;
@@ -402,10 +414,11 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->probe = 0;
   h->accumulate = 0;
   h->acc_count = 0;
-  h->opt_diag_plan = 0; h->opt_pairs = 1; h->opt_wide = 1; h->opt_units = 0; h->opt_f32_generic = 0; h->opt_pdl = 1;
+  h->opt_diag_plan = 0; h->opt_pairs = 1; h->opt_wide = 1; h->opt_units = 0; h->opt_f32_generic = 0; h->opt_pdl = 1; h->opt_collect = 1; h->opt_resident = 1;
   h->d_items_f32 = nullptr;
   h->d_scratch = nullptr;
   h->d_wide_vis = nullptr;
+  h->d_diag_stats = nullptr;
   h->d_stream_in[0] = h->d_stream_in[1] = nullptr;
   h->s_copy = h->s_compute = nullptr;
 
@@ -437,6 +450,7 @@ int corr_destroy(corr_handle *h) {
   cudaFree(h->d_items_f32);
   cudaFree(h->d_scratch);
   cudaFree(h->d_wide_vis);
+  cudaFree(h->d_diag_stats);
   cudaFree(h->d_stream_in[0]);
   cudaFree(h->d_stream_in[1]);
   if (h->s_copy) cudaStreamDestroy(h->s_copy);
@@ -464,7 +478,9 @@ int corr_set_option(corr_handle *h, int key, int value) {
       break;
     }
     case CORR_OPT_PAIRS: h->opt_pairs = value ? 1 : 0; break;
-    case CORR_OPT_WIDE: h->opt_wide = value ? 1 : 0; break;
+    case CORR_OPT_WIDE: h->opt_wide = value < 0 ? 0 : (value > 2 ? 2 : value); break;
+    case CORR_OPT_COLLECT: h->opt_collect = value ? 1 : 0; break;
+    case CORR_OPT_RESIDENT: h->opt_resident = value ? 1 : 0; break;
     case CORR_OPT_UNITS:
       if (value < 0) return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_UNITS must be >= 0");
       h->opt_units = value;
@@ -583,6 +599,26 @@ int corr_probe_ffma(int packed, int iters, double *out) {
 int corr_set_probe(corr_handle *h, int mode) {
   if (!h) return fail(CORR_EINVAL, "corr_set_probe: NULL handle");
   h->probe = mode;
+  if ((mode & ~128) && h->dtype != CORR_CF32 && h->plan.ip.resident) {
+    // the engine switches live in the streaming producers / issuer only: fall back to the streaming pair plan
+    h->opt_resident = 0;
+    if (int rc = replan(h)) return rc;
+  }
+  if ((mode & 128) && !h->d_diag_stats) {
+    CUDA_TRY(cudaMalloc(&h->d_diag_stats, 4 * 256 * sizeof(unsigned long long)));
+    CUDA_TRY(cudaMemset(h->d_diag_stats, 0, 4 * 256 * sizeof(unsigned long long)));
+  }
+  return CORR_OK;
+}
+
+int corr_probe_stats(corr_handle *h, double *out) {
+  if (!h || !out || !h->d_diag_stats) return fail(CORR_EINVAL, "corr_probe_stats: no statistics (corr_set_probe(h, 128) first)");
+  const int units = h->plan.ip.units;
+  std::vector<unsigned long long> st(4 * 256);
+  CUDA_TRY(cudaMemcpy(st.data(), h->d_diag_stats, st.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  for (int k = 0; k < 4; ++k) out[k] = 0.0;
+  for (int u = 0; u < units; ++u)
+    for (int k = 0; k < 4; ++k) out[k] += static_cast<double>(st[4 * u + k]) / units;
   return CORR_OK;
 }
 #endif  // CORR_DIAG
@@ -662,8 +698,7 @@ int corr_set_turn(corr_handle *h, int mode) {
     }
   }
   h->turn_mode = mode;
-  h->maps.clear();
-  return CORR_OK;
+  return replan(h);  // the resident-A plan reads d_in through 2-D maps only: the standalone turn takes the streaming plan
 }
 
 static int launch_turn(corr_handle *h, const void *d_in, void *d_out, cudaStream_t st) {
@@ -769,8 +804,10 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.turned = turned ? 1 : 0;
   ip.vis = static_cast<int2 *>(d_vis);
   ip.probe = h->probe;
+  ip.diag_stats = h->d_diag_stats;
   ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
   ip.accumulate = h->accumulate;
+  ip.collect = h->opt_collect;
   if (ip.n_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
   if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<grid, corr::kI4Threads, smem, st>>>(*maps, ip);
   else if (ip.pair2) corr::xengine_i8_pair_kernel<<<grid, corr::kI8Threads, smem, st>>>(*maps, ip);

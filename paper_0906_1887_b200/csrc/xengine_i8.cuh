@@ -63,8 +63,13 @@ struct I8Params {
   int stages, stage_bytes;
   int turned;        // 0: d_in is [T][C][2N] (2-D maps); 1: scratch is [G][T][W] (3-D maps)
   int probe;         // diagnostics only (corr_set_probe)
+  unsigned long long *diag_stats;  // diagnostics only (probe bit 128): [unit][4] = kernel cycles, MMA waits for loads, MMA waits for TMEM, producer waits for a stage
   int out_shift;     // 8 for 4-bit input (operands are 16 x the samples), else 0
   int accumulate;    // 1: add this integration into d_vis instead of overwriting it
+  int resident;      // 1: CTA pairs keep their A panel of the WHOLE integration in shared memory (T <= 1024) and walk all
+                     //    column tiles of a row pair with it; an item is then a unit of two row pairs (xengine_i8_resident.cuh)
+  int a_sub;         // resident: 128-row sub-stages of the A region (ceil(T / 128))
+  int collect;       // 1: 512-wide pair tiles issue their two MMAs per k-step with A-collector reuse
   long long n_baselines;
   int2 *vis;
   unsigned short kinds[kMaxKinds];  // slab: I | (J0 / 2) << 6 | (nblk - 1) << 11; pair: Ip | (J0 / 2) << 6 | wide << 11
@@ -178,6 +183,39 @@ __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c
   if (it.n_load * 256 * kPanelBytes <= p.stage_bytes)      { it.bk = 256; it.map = 0; }
   else if (it.n_load * 128 * kPanelBytes <= p.stage_bytes) { it.bk = 128; it.map = 1; }
   else                                                     { it.bk = 64;  it.map = 2; }
+  return it;
+}
+
+// Resident-A plans: the tiles of one schedule item (a unit = row pairs R1 = pp-1-u and R2 = u of one channel, so that
+// every unit has pp + 1 tiles), in the order every role walks them: row R1 first, each row's column tiles J0 = 0, 2, ...
+// with the diagonal tile (J0 = 2R, whose B operand IS the resident A panel) last.
+struct ResTile {
+  int R, J0;
+  bool first, diag;  // first / last (diagonal) tile of its row
+};
+__device__ __forceinline__ int res_n_tiles(const I8Params &p, const I8Iter &c) {
+  const int pp = (p.n_panels + 1) >> 1, u = c.k, r1 = pp - 1 - u;
+  return (r1 + 1) + (r1 != u ? u + 1 : 0);
+}
+__device__ __forceinline__ ResTile res_tile(const I8Params &p, const I8Iter &c, int sub) {
+  const int pp = (p.n_panels + 1) >> 1, u = c.k, r1 = pp - 1 - u;
+  ResTile t;
+  if (sub <= r1) { t.R = r1; t.J0 = 2 * sub; }
+  else           { t.R = u;  t.J0 = 2 * (sub - r1 - 1); }
+  t.first = t.J0 == 0;
+  t.diag = t.J0 == 2 * t.R;
+  return t;
+}
+__device__ __forceinline__ I8Item res_item(const I8Params &p, const I8Iter &c, const ResTile &t, int rank) {
+  I8Item it;
+  it.t0 = 0; it.t1 = p.n_time;
+  it.nblk = 2; it.nblk_load = 1; it.jperm = 0; it.n_load = t.diag ? 0 : 1; it.a_slot = 0;
+  it.chan = c.grp; it.I = 2 * t.R + rank; it.J0 = t.J0;
+  it.dx = kPanelBytes; it.dz = 0; it.z0 = 0; it.za = 0;
+  const int xc = c.grp * 2 * p.n_inputs;
+  it.x0 = xc + (t.J0 + rank) * kPanelBytes;
+  it.xa = xc + it.I * kPanelBytes;
+  it.bk = 128; it.map = 1;
   return it;
 }
 

@@ -17,6 +17,31 @@ __device__ __forceinline__ void issue_k(uint32_t d, uint32_t lo_a, uint32_t lo_b
     else       mma_i8_ss(d, da, db, idesc, k == 0 ? acc0 : 1u);
   }
 }
+// 512-wide pair tiles: per k-step the same A tile multiplies two B tiles (column halves d0, d1).  Issued back to
+// back with collector hints, so that the tensor core reads A from shared memory once per k-step instead of twice.
+template <int NK>
+__device__ __forceinline__ void issue_k_wide(uint32_t d0, uint32_t d1, uint32_t lo_a, uint32_t lo_b0, uint32_t lo_b1,
+                                             uint32_t hi, uint32_t idesc, uint32_t acc0) {
+#pragma unroll
+  for (int k = 0; k < NK; ++k) {
+    const uint64_t da = (static_cast<uint64_t>(hi) << 32) | (lo_a + k * (32 * kPanelBytes / 16));
+    const uint64_t db0 = (static_cast<uint64_t>(hi) << 32) | (lo_b0 + k * (32 * kPanelBytes / 16));
+    const uint64_t db1 = (static_cast<uint64_t>(hi) << 32) | (lo_b1 + k * (32 * kPanelBytes / 16));
+    mma_i8_ss_2sm_collect<1>(d0, da, db0, idesc, k == 0 ? acc0 : 1u);
+    mma_i8_ss_2sm_collect<2>(d1, da, db1, idesc, k == 0 ? acc0 : 1u);
+  }
+}
+__device__ __forceinline__ void issue_kn_wide(uint32_t d0, uint32_t d1, uint32_t lo_a, uint32_t lo_b0, uint32_t lo_b1,
+                                              uint32_t hi, uint32_t idesc, uint32_t acc0, int nk) {
+  for (int k = 0; k < nk; ++k) {
+    const uint64_t da = (static_cast<uint64_t>(hi) << 32) | (lo_a + k * (32 * kPanelBytes / 16));
+    const uint64_t db0 = (static_cast<uint64_t>(hi) << 32) | (lo_b0 + k * (32 * kPanelBytes / 16));
+    const uint64_t db1 = (static_cast<uint64_t>(hi) << 32) | (lo_b1 + k * (32 * kPanelBytes / 16));
+    mma_i8_ss_2sm_collect<1>(d0, da, db0, idesc, k == 0 ? acc0 : 1u);
+    mma_i8_ss_2sm_collect<2>(d1, da, db1, idesc, k == 0 ? acc0 : 1u);
+  }
+}
+
 template <bool kPair>
 __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_b, uint32_t hi, uint32_t idesc,
                                          uint32_t acc0, int nk) {
@@ -30,6 +55,10 @@ __device__ __forceinline__ void issue_kn(uint32_t d, uint32_t lo_a, uint32_t lo_
 
 // maps: the tensor maps of the input(s), [n_batch][3] (box heights 256 / 128 / 64 time rows); vis_list: the output of
 // every integration of a batched launch (kBatch), else unused (p.vis).
+}  // namespace corr
+#include "xengine_i8_resident.cuh"
+namespace corr {
+
 template <bool kPair, bool kProbe, bool kPacked = false, bool kBatch = false>
 __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *const *vis_list, const I8Params &p) {
   // All shared memory is dynamic (no static variables), so the window starts 1024-byte aligned as the
@@ -37,8 +66,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   extern __shared__ __align__(1024) uint8_t smem[];
   // 4-bit packed input (kPacked): TMA lands the packed boxes in a second ring (half the bytes) behind the
   // int8 ring; four expand warps sign-extend the nibbles into the int8 ring in the MN-major SW128 layout.
+  // Resident-A plans (CTA pairs, T <= 1024) put the A panel of the whole integration in front of the ring.
+  const uint32_t a_bytes = (kPair && p.resident) ? static_cast<uint32_t>(p.a_sub) * kResSubBytes : 0;
+  uint8_t *ring_base = smem + a_bytes;
   const uint32_t raw_stage_bytes = kPacked ? static_cast<uint32_t>(p.stage_bytes) / 2 : 0;
-  uint8_t *raw = smem + static_cast<size_t>(p.stages) * p.stage_bytes;
+  uint8_t *raw = ring_base + static_cast<size_t>(p.stages) * p.stage_bytes;
   uint8_t *epi_stage = raw + static_cast<size_t>(p.stages) * raw_stage_bytes;
   uint64_t *full_bar = reinterpret_cast<uint64_t *>(epi_stage + kEpiWarps * kEpiWarpBytes);
   uint64_t *empty_bar = full_bar + kMaxStages;
@@ -46,7 +78,9 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   uint64_t *acc_empty = acc_full + 2;
   uint64_t *raw_full = acc_empty + 2;
   uint64_t *raw_empty = raw_full + kMaxStages;
-  uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(raw_empty + kMaxStages);
+  uint64_t *a_full = raw_empty + kMaxStages;  // resident-A plans: one pair of barriers per 128-row sub-stage of the A region
+  uint64_t *a_empty = a_full + kResMaxSub;
+  uint32_t &tmem_base_smem = *reinterpret_cast<uint32_t *>(a_empty + kResMaxSub);
 
   // programmatic dependent launch (single-CTA kernels): the next call's launch, barrier set-up and TMEM allocation may
   // overlap this call's tail; every role that touches global memory waits for the preceding grid first
@@ -72,6 +106,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
         mbar_init(&raw_empty[s], kExpandWarps);
       }
     }
+    if (kPair)
+      for (int g = 0; g < kResMaxSub; ++g) {
+        mbar_init(&a_full[g], 1);
+        mbar_init(&a_empty[g], 1);
+      }
     for (int r = 0; r < 2; ++r) {
       mbar_init(&acc_full[r], 1);
       mbar_init(&acc_empty[r], kEpiWarps * (kPair ? 2 : 1));  // one arrive per epilogue warp (of both CTAs)
@@ -84,7 +123,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
 
-  if (warp == kProducerWarp || warp == kProducerWarp2) {
+  if (kPair && p.resident && (warp == kProducerWarp || warp == kProducerWarp2 || warp == kMmaWarp)) {
+    // ===================================================================== resident-A plans: their own producers and issuer
+    if (warp == kMmaWarp) resident_mma<kProbe>(p, smem, a_bytes, full_bar, empty_bar, acc_full, acc_empty, a_full, a_empty, tmem_base, n_rounds, rank);
+    else resident_producer(p, maps, smem, a_bytes, full_bar, empty_bar, a_full, a_empty, n_rounds, rank, warp == kProducerWarp2);
+  } else if (warp == kProducerWarp || warp == kProducerWarp2) {
     // ===================================================================== TMA producers
     // two warps walk the same schedule and take alternate stages: one thread cannot issue the boxes of a
     // stage (wait, expect_tx, up to 4 TMA instructions) as fast as the tensor pipe drains it
@@ -96,6 +139,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
       const uint32_t full_leader = kPair ? mapa_u32(&full_bar[0], 0) : 0;
       int stage = 0;
       uint32_t phase = 0;
+      long long w_empty = 0;  // diagnostics (probe bit 128): cycles this producer waited for a free stage
       I8Iter cur = iter_init(p);
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
@@ -121,13 +165,16 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
             if (++stage == p.stages) { stage = 0; phase ^= 1; }
             continue;
           }
+          long long tw = 0;
+          if (kProbe && (probe & 128)) tw = clock64();
           mbar_wait(&empty_bar[stage], phase ^ 1);
+          if (kProbe && (probe & 128)) w_empty += clock64() - tw;
           if (probe & 2) {
             if (rank == 0) mbar_arrive(&full_bar[stage]);
           } else {
             // pair mode: both CTAs' boxes complete on the LEADER's barrier, which expects the bytes of both
             if (rank == 0) mbar_expect_tx(&full_bar[stage], panel_bytes * it.n_load * (kPair ? 2 : 1));
-            uint8_t *dst = smem + static_cast<size_t>(stage) * p.stage_bytes;
+            uint8_t *dst = ring_base + static_cast<size_t>(stage) * p.stage_bytes;
             const uint32_t bar2 = kPair ? full_leader + stage * 8 : 0;
             for (int l = 0; l < it.n_load; ++l) {
               const bool is_a = l >= it.nblk_load;
@@ -145,6 +192,8 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
         }
       }
+      if (kProbe && (probe & 128) && p.diag_stats && rank == 0 && pw == 0)
+        p.diag_stats[4 * (blockIdx.x >> (kPair ? 1 : 0)) + 3] = static_cast<unsigned long long>(w_empty);
     }
   } else if (warp == kMmaWarp) {
     // ===================================================================== MMA issuer
@@ -159,8 +208,10 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
       constexpr uint32_t kIdesc128 = idesc_i8_mn(128, 128);
       constexpr uint32_t kIdesc256 = kPair ? idesc_i8_mn(256, 256) : idesc_i8_mn(128, 256);
       constexpr uint32_t kDescHi = static_cast<uint32_t>(((1024ull >> 4) | (1ull << 14) | (2ull << 29)));
-      const uint32_t smem_lo = (smem_u32(smem) & 0x3FFFFu) >> 4;
+      const uint32_t smem_lo = (smem_u32(ring_base) & 0x3FFFFu) >> 4;
       const uint32_t tmem_u = tmem_base;
+      long long w_full = 0, w_acc = 0, t_begin = 0;  // diagnostics (probe bit 128): cycles spent waiting for loads / for TMEM
+      if (kProbe && (probe & 128)) t_begin = clock64();
       I8Iter cur = iter_init(p);
       for (int r = 0; r < n_rounds; ++r, iter_next(p, cur)) {
         if (!iter_valid(p, cur)) continue;
@@ -173,14 +224,19 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
         const uint32_t a_off = static_cast<uint32_t>(it.a_slot) * panel16;
         const uint32_t lbo_field = (panel16 & 0x3FFFu) << 16;
         const int n_chunks = (u_nblk + 1) >> 1;
+        long long tw = 0;
+        if (kProbe && (probe & 128)) tw = clock64();
         if (!(probe & 4))
           for (int q = 0; q < n_chunks; ++q) mbar_wait(&acc_empty[(ring + q) & 1], (((ring + q) >> 1) & 1) ^ 1);
+        if (kProbe && (probe & 128)) w_acc += clock64() - tw;
         tc_fence_after();
         const uint32_t d0 = tmem_u + (ring & 1) * kAccCols;        // chunk 0
         const uint32_t d1 = tmem_u + ((ring + 1) & 1) * kAccCols;  // chunk 1
         const uint32_t idesc0 = u_nblk >= 2 ? kIdesc256 : kIdesc128;
         for (int t = u_t0; t < u_t1; t += u_bk) {
+          if (kProbe && (probe & 128)) tw = clock64();
           if (!(probe & 8)) mbar_wait(&full_bar[stage], phase);
+          if (kProbe && (probe & 128)) w_full += clock64() - tw;
           if (!(kProbe && (probe & 64))) tc_fence_after();
           const uint32_t lo_stage = (smem_lo + static_cast<uint32_t>(stage) * (p.stage_bytes >> 4)) | lbo_field;
           const int nk = (min(u_bk, u_t1 - t) + 31) >> 5;  // K = 32 samples per MMA; TMA zero-fills past T
@@ -195,7 +251,11 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
               }
             } else {
               const uint32_t lo_a = lo_stage + a_off;
-              if (kProbe && (probe & 32) && nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);  // diagnostics: issue twice
+              if (kPair && u_nblk > 2 && p.collect) {  // 512-wide pair tile, A read once per k-step (collector reuse)
+                const uint32_t lo_b1 = lo_stage + panel16;
+                if (nk == 4) issue_k_wide<4>(d0, d1, lo_a, lo_stage, lo_b1, kDescHi, idesc0, acc0);
+                else         issue_kn_wide(d0, d1, lo_a, lo_stage, lo_b1, kDescHi, idesc0, acc0, nk);
+              } else {
               if (nk == 2)      issue_k<2, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else if (nk == 4) issue_k<4, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
               else if (nk == 8) issue_k<8, kPair>(d0, lo_a, lo_stage, kDescHi, idesc0, acc0);
@@ -204,6 +264,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
                 const uint32_t lo_b1 = lo_stage + panel16;
                 if (nk == 4) issue_k<4, kPair>(d1, lo_a, lo_b1, kDescHi, idesc0, acc0);
                 else         issue_kn<kPair>(d1, lo_a, lo_b1, kDescHi, idesc0, acc0, nk);
+              }
               }
             }
           }
@@ -217,6 +278,12 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
             if (kPair) mma_commit_2sm(&acc_full[(ring + q) & 1], 3); else mma_commit(&acc_full[(ring + q) & 1]);
           }
         ring += n_chunks;
+      }
+      if (kProbe && (probe & 128) && p.diag_stats) {
+        unsigned long long *st = p.diag_stats + 4 * (blockIdx.x >> (kPair ? 1 : 0));
+        st[0] = static_cast<unsigned long long>(clock64() - t_begin);
+        st[1] = static_cast<unsigned long long>(w_full);
+        st[2] = static_cast<unsigned long long>(w_acc);
       }
     }
   } else if (kPacked && warp >= kExpandWarp0) {
@@ -240,7 +307,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
         mbar_wait(&raw_full[stage], phase);       // packed bytes have landed
         mbar_wait(&empty_bar[stage], phase ^ 1);  // the int8 slot has been consumed by the MMAs
         const uint8_t *src = raw + static_cast<size_t>(stage) * raw_stage_bytes;
-        uint8_t *dst = smem + static_cast<size_t>(stage) * p.stage_bytes;
+        uint8_t *dst = ring_base + static_cast<size_t>(stage) * p.stage_bytes;
         for (int idx = et; idx < n_chunks; idx += kExpandWarps * 32) {
           const int l = idx >> sh;            // panel (bk * 4 chunks each, a power of two)
           const int rem = idx & ((1 << sh) - 1);
@@ -276,10 +343,10 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
     constexpr int kShift = kPacked ? 8 : 0;
     if (p.n_slices > 1 || p.accumulate)
-      i8_epilogue<true, kShift, kBatch>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+      i8_epilogue<true, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
                                         acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
     else
-      i8_epilogue<false, kShift, kBatch>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+      i8_epilogue<false, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
                                          acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 

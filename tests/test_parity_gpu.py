@@ -70,6 +70,10 @@ CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (
               (512, 3, 200), (576, 2, 70), (512, 40, 33), (2048, 1, 64),
               # long integrations (T >= 2048): 512-wide pair tiles from N_I = 256 up, mixed with 256-wide ones
               (256, 3, 2100), (320, 1, 2050), (512, 1, 2081),
+              # resident-A plans (N_I >= 512, T <= 1024): full-length A region, ragged last sub-stage, odd panel count
+              (512, 2, 1000), (640, 3, 1024), (576, 5, 129), (1024, 2, 300),
+              # CTA pairs without the resident plan: 1024 < T < 2048
+              (512, 1, 1100),
               # the largest N_I the ABI admits (528 schedule kinds per channel)
               (4096, 1, 40)]
 
@@ -94,6 +98,21 @@ def test_ci8_single_cta_slabs_when_pairs_are_disabled(pkg, N, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
     assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_PAIRS, 0)]), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("N,C,T", [(512, 3, 200), (576, 2, 70), (1024, 1, 96), (512, 2, 1000)])
+def test_ci8_pair_tiles_without_the_resident_plan(pkg, N, C, T):
+    """corr_set_option(CORR_OPT_RESIDENT, 0): N_I >= 512, T <= 1024 on the streaming 256 x 256 pair tiles."""
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_RESIDENT, 0)]), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (512, 1, 2081)])
+def test_ci8_wide_pair_tiles_without_collector_reuse(pkg, N, C, T):
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_COLLECT, 0)]), oracle.xengine_ci8(x, threads=_threads()))
 
 
 @pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (512, 1, 2081)])
