@@ -741,6 +741,11 @@ def main():
             "e2e": e2e, "gpu_launches": r["launches"], "roofline": roof}
     if not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(w, gpu_vis=gpu_vis)
+    if args.config in ("c2", "c4") and world == 1 and not args.no_sweep:
+        try:   # the standalone corner turn (a1, second realisation) measured on the headline workload
+            line["corner_turn"] = corner_turn_entry(pkg, torch, w, h, r["bufs"][0])
+        except Exception as e:
+            line["corner_turn"] = {"error": str(e)[:200]}
     del r
     h.destroy()
     torch.cuda.empty_cache()

@@ -175,6 +175,16 @@ __host__ __device__ constexpr uint32_t idesc_i8_mn(uint32_t M, uint32_t N) {
 
 }  // namespace corr
 
+// ----------------------------------------------------------------------------- bulk async loads
+namespace corr {
+// global -> shared::cta, contiguous, 16-byte aligned on both sides, size a multiple of 16; completes `bar` with the bytes
+__device__ __forceinline__ void bulk_load(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+}  // namespace corr
+
 // ----------------------------------------------------------------------------- bulk async stores
 namespace corr {
 // shared::cta -> global, 16-byte aligned on both sides, size a multiple of 16; joins the bulk async-group

@@ -14,7 +14,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "xengine_f32.cuh"  // cp_async16 / commit / wait
+#include "ptx_sm100.cuh"    // mbarrier, cp.async.bulk
+#include "xengine_f32.cuh"
 
 namespace corr {
 
@@ -24,7 +25,8 @@ constexpr int kN64Threads = kN64Chan * kN64Tiles;  // 504
 constexpr int kN64TB = 16;                     // time rows per stage
 constexpr int kN64Stages = 3;
 constexpr int kN64RowF4 = kN64Chan * 32;       // float4 per time row of a group (3.5 KB)
-constexpr int kN64Smem = kN64Stages * kN64TB * kN64RowF4 * 16;  // 168 KB
+constexpr int kN64Warps = (kN64Threads + 31) / 32;               // 16
+constexpr int kN64Smem = kN64Stages * kN64TB * kN64RowF4 * 16 + 64;  // 168 KB + the stage barriers
 
 struct F32N64Params {
   const float2 *in;  // [T][C][64]
@@ -68,15 +70,28 @@ __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F
   const float4 *src0 = reinterpret_cast<const float4 *>(p.in) + static_cast<long long>(p.chan0 + c0) * 32;
   const int valid_f4 = n_chan_here * 32;
 
-  auto load_stage = [&](int s) {
-    float4 *dst = n64_smem + (s % kN64Stages) * (kN64TB * kN64RowF4);
-    const int tb = t0 + s * kN64TB;
-    for (int idx = tid; idx < kN64TB * kN64RowF4; idx += kN64Threads) {
-      const int r = idx / kN64RowF4, k = idx - r * kN64RowF4;
-      const int t = tb + r;
-      const bool ok = (t < t1) && (k < valid_f4);
-      cp_async16(dst + idx, src0 + (ok ? static_cast<long long>(t) * row_f4 + k : 0), ok);
+  // Stage pipeline: one thread feeds a ring of kN64Stages stages with bulk copies (one contiguous 3.5 KB run per time
+  // row) that complete on the stage's `full` mbarrier; every warp arrives on the stage's `empty` mbarrier when it has
+  // consumed it.  No CTA-wide barrier in the loop: warps drift up to two stages apart instead of meeting 32 times.
+  uint64_t *full_bar = reinterpret_cast<uint64_t *>(n64_smem + kN64Stages * kN64TB * kN64RowF4);
+  uint64_t *empty_bar = full_bar + kN64Stages;
+  if (tid == 0) {
+    for (int s = 0; s < kN64Stages; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], kN64Warps);
     }
+    fence_mbar_init();
+  }
+  __syncthreads();
+  const uint32_t row_bytes = static_cast<uint32_t>(valid_f4) * 16;
+  auto load_stage = [&](int s) {  // thread 0 only
+    const int slot = s % kN64Stages;
+    float4 *dst = n64_smem + slot * (kN64TB * kN64RowF4);
+    const int tb = t0 + s * kN64TB;
+    const int rows = min(kN64TB, t1 - tb);
+    mbar_expect_tx(&full_bar[slot], rows * row_bytes);
+    for (int r = 0; r < rows; ++r)
+      bulk_load(dst + r * kN64RowF4, src0 + static_cast<long long>(tb + r) * row_f4, row_bytes, &full_bar[slot]);
   };
 
   float2 acc[8][4];  // (Re, Im) of V_ij, i = 8 ti + a, j = this thread's b-th column
@@ -86,21 +101,25 @@ __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F
     for (int b = 0; b < 4; ++b) acc[a][b] = make_float2(0.f, 0.f);
 
   const int n_stages = (t1 - t0 + kN64TB - 1) / kN64TB;
-  load_stage(0);
-  cp_async_commit();
-  if (n_stages > 1) load_stage(1);
-  cp_async_commit();
+  if (tid == 0)
+    for (int s = 0; s < min(kN64Stages, n_stages); ++s) load_stage(s);
 
   const int off_i = cg * 32 + 4 * ti;
   const int off_j0 = cg * 32 + 2 * tj + sw, off_j1 = cg * 32 + 2 * tj + 1 - sw;
   for (int s = 0; s < n_stages; ++s) {
-    cp_async_wait<1>();   // stage s has landed (at most the group of stage s + 1 is still in flight)
-    __syncthreads();      // ... for every thread, and everyone has finished computing stage s - 1
-    if (s + 2 < n_stages) load_stage(s + 2);  // into the buffer stage s - 1 used
-    cp_async_commit();
-    const float4 *st = n64_smem + (s % kN64Stages) * (kN64TB * kN64RowF4);
+    const int slot = s % kN64Stages;
+    const uint32_t par = (s / kN64Stages) & 1;
+    // refill the slot of the PREVIOUS stage (the other warps have had a whole stage's time to leave it, so this wait
+    // rarely blocks) with the stage two ahead of this one
+    if (tid == 0 && s >= 1 && s - 1 + kN64Stages < n_stages) {
+      mbar_wait(&empty_bar[(s - 1) % kN64Stages], ((s - 1) / kN64Stages) & 1);
+      load_stage(s - 1 + kN64Stages);
+    }
+    mbar_wait(&full_bar[slot], par);  // the stage's rows have landed
+    const float4 *st = n64_smem + slot * (kN64TB * kN64RowF4);
+    const int rows = min(kN64TB, t1 - (t0 + s * kN64TB));
 #pragma unroll 2
-    for (int r = 0; r < kN64TB; ++r) {
+    for (int r = 0; r < rows; ++r) {
       const float4 *row = st + r * kN64RowF4;
       const float4 a0 = row[off_i], a1 = row[off_i + 1], a2 = row[off_i + 2], a3 = row[off_i + 3];
       const float4 b0 = row[off_j0], b1 = row[off_j1];
@@ -122,6 +141,9 @@ __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F
         }
       }
     }
+    // this warp is done with the stage
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(&empty_bar[slot]);
   }
 
   if (active) {
