@@ -243,6 +243,8 @@ size_t corr_fstage_out_bytes(const corr_fstage *f); /* n_batch * n_fft * n_input
  *   h_raw : n_integrations pointers to PINNED host buffers of corr_fstage_in_bytes(f) bytes
  *   d_vis, stats : as corr_stream_run ([2] = sum of F + X kernel seconds).
  * The F-stage handle owns two raw buffers and one spectra buffer on the device from the first call on.
+ * Tolerance of the chain against float64 arithmetic on the same raw voltages: |dV| <= 2e-5 sqrt(|V_ii V_jj|) --
+ * two FP32 stages in a row, each good to 1e-5 of its own scale.
  */
 int corr_stream_run_fx(corr_handle *h, corr_fstage *f, const void *const *h_raw, int n_integrations,
                        void *d_vis, double *stats);
