@@ -65,7 +65,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   // 128-byte swizzle needs: [stage ring][epilogue staging][mbarriers + TMEM base].
   extern __shared__ __align__(1024) uint8_t smem[];
   // 4-bit packed input (kPacked): TMA lands the packed boxes in a second ring (half the bytes) behind the
-  // int8 ring; four expand warps sign-extend the nibbles into the int8 ring in the MN-major SW128 layout.
+  // int8 ring; eight expand warps sign-extend the nibbles into the int8 ring in the MN-major SW128 layout.
   // Resident-A plans (CTA pairs, T <= 1024) put the A panel of the whole integration in front of the ring.
   const uint32_t a_bytes = (kPair && p.resident) ? static_cast<uint32_t>(p.a_sub) * kResSubBytes : 0;
   uint8_t *ring_base = smem + a_bytes;
@@ -91,7 +91,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   const int n_rounds = (p.n_items + p.units - 1) / p.units;
   const int rank = kPair ? static_cast<int>(cluster_ctarank()) : 0;  // CTA within the pair; 0 issues the MMAs
 
-  // Warp roles: epilogue = warps 0-7, TMA producer = 8, MMA issuer = 9, TMEM allocator = 10.  The single-thread
+  // Warp roles: epilogue = warps 0-7, TMA producers = 8 and 11, MMA issuer = 9, TMEM allocator = 10.  The single-thread
   // roles sit in the HIGHEST warps because the SMSP arbiter favours higher warp ids: they are the critical
   // path and must not queue behind eight busy epilogue warps.
   if (warp == kProducerWarp && lane == 0) {
