@@ -105,7 +105,7 @@ struct corr_handle {
   int2 *d_items_f32;
   int n_items_f32;
   int f32_threads;
-  int n64_groups, n64_slices, n64_slice_len;  // CF32 with N_I = 64: xengine_f32_n64_kernel
+  int n64_groups, n64_slices, n64_slice_len, n64_full;  // CF32 with N_I = 64: xengine_f32_n64_kernel
   // streaming driver
   void *d_stream_in[2];
   cudaStream_t s_copy, s_compute;
@@ -267,17 +267,30 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
   h->n_items_f32 = static_cast<int>(items.size());
   // N_I = 64: (8-channel group, time slice) units; as many slices as fill the SMs evenly (cost = rounds x rows per
   // slice, plus 32 rows for the zeroing node and the reduce-adds of a sliced plan)
-  h->n64_groups = h->n64_slices = h->n64_slice_len = 0;
+  h->n64_groups = h->n64_slices = h->n64_slice_len = h->n64_full = 0;
   if (h->n_inputs == 64 && !h->opt_f32_generic) {
     const int T = h->n_time, G = h->n_sms;
     h->n64_groups = (h->n_chan + corr::kN64Chan - 1) / corr::kN64Chan;
+    // (A) every group cut into the same number of slices: cost = rounds x rows per slice (+ 32 rows for the zeroing
+    // node and the reduce-adds of a sliced plan)
     long long best = -1;
     for (int sl = 1; sl <= 32; ++sl) {
       const int len = ((T + sl - 1) / sl + corr::kN64TB - 1) / corr::kN64TB * corr::kN64TB;
       if ((T + len - 1) / len != sl) continue;
       const long long rounds = (1LL * h->n64_groups * sl + G - 1) / G;
       const long long cost = rounds * len + (sl > 1 ? 32 : 0);
-      if (best < 0 || cost < best) { best = cost; h->n64_slices = sl; h->n64_slice_len = len; }
+      if (best < 0 || cost < best) { best = cost; h->n64_slices = sl; h->n64_slice_len = len; h->n64_full = 0; }
+    }
+    // (B) a x G whole groups (a per SM, plain stores, no zeroing) and only the b left-over groups cut into G / b
+    // slices: fewer CTAs, and the zeroing node covers the sliced groups' channels only (c5: 148 whole groups + 72
+    // groups in halves instead of 220 groups in halves)
+    const int a = h->n64_groups / G, b = h->n64_groups % G;
+    if (a >= 1 && b > 0) {
+      int sl = std::min(32, G / b);
+      int len = ((T + sl - 1) / sl + corr::kN64TB - 1) / corr::kN64TB * corr::kN64TB;
+      sl = (T + len - 1) / len;
+      const long long cost = 1LL * a * T + len + (sl > 1 ? 8 : 0) - 16;  // one CTA start-up per SM less than (A)
+      if (sl > 1 && cost < best) { best = cost; h->n64_slices = sl; h->n64_slice_len = len; h->n64_full = a * G; }
     }
   }
   h->f32_threads = blocks == 1 ? 160 : corr::kF32Threads;  // 136 active tiles on a diagonal block
@@ -764,9 +777,15 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
       np.n_time = h->n_time; np.n_chan = h->n_chan;
       np.n_chan_total = h->n_chan_total; np.chan0 = h->chan0;
       np.n_groups = h->n64_groups; np.n_slices = h->n64_slices; np.slice_len = h->n64_slice_len;
-      np.add = (h->n64_slices > 1 || h->accumulate) ? 1 : 0;
-      if (h->n64_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));
-      corr::xengine_f32_n64_kernel<<<h->n64_groups * h->n64_slices, corr::kN64Threads, corr::kN64Smem, st>>>(np);
+      np.n_full = h->n64_full;
+      np.add = h->accumulate ? 1 : 0;
+      if (h->n64_slices > 1 && !h->accumulate) {  // the sliced groups' channels are zeroed: their slices reduce-add
+        const size_t chan0 = static_cast<size_t>(h->n64_full) * corr::kN64Chan;
+        const size_t off = chan0 * h->n_baselines * 8;
+        CUDA_TRY(cudaMemsetAsync(static_cast<char *>(d_vis) + off, 0, h->vis_bytes - off, st));
+      }
+      const int units = h->n64_full + (h->n64_groups - h->n64_full) * h->n64_slices;
+      corr::xengine_f32_n64_kernel<<<units, corr::kN64Threads, corr::kN64Smem, st>>>(np);
       CUDA_TRY(cudaGetLastError());
       if (h->accumulate) ++h->acc_count;
       return CORR_OK;

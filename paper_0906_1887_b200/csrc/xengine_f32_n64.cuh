@@ -32,8 +32,10 @@ struct F32N64Params {
   const float2 *in;  // [T][C][64]
   float2 *vis;       // [C][2080]
   int n_time, n_chan, n_groups, n_slices, slice_len;
+  int n_full;        // the first n_full groups are whole integrations (one unit each, plain stores); the other
+                     // n_groups - n_full groups are cut into n_slices time slices that reduce-add into zeroed output
   int n_chan_total, chan0;  // d_in is [T][n_chan_total][64]; this handle correlates channels chan0 .. chan0 + n_chan - 1
-  int add;           // 1: reduce-add into d_vis (time slices or accumulate mode); 0: plain stores
+  int add;           // 1: accumulate mode, every unit reduce-adds into d_vis; 0: only the units of sliced groups do
 };
 
 __device__ __forceinline__ void red_add_f32x2(float2 *dst, float re, float im) {
@@ -48,10 +50,19 @@ __device__ __forceinline__ void ffma2(float2 &acc, const float2 &a, const float2
 __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F32N64Params p) {
   extern __shared__ __align__(16) float4 n64_smem[];
   const int tid = threadIdx.x;
-  const int grp = blockIdx.x % p.n_groups;
-  const int slice = blockIdx.x / p.n_groups;
-  const int t0 = slice * p.slice_len;
-  const int t1 = min(p.n_time, t0 + p.slice_len);
+  // units: the whole groups first (they are the long ones), then the slices of the sliced groups
+  int grp, t0, t1;
+  bool add = p.add != 0;
+  if (static_cast<int>(blockIdx.x) < p.n_full) {
+    grp = blockIdx.x; t0 = 0; t1 = p.n_time;
+  } else {
+    const int u = static_cast<int>(blockIdx.x) - p.n_full;
+    const int n_cut = p.n_groups - p.n_full;
+    grp = p.n_full + u % n_cut;
+    t0 = (u / n_cut) * p.slice_len;
+    t1 = min(p.n_time, t0 + p.slice_len);
+    add = add || p.n_slices > 1;
+  }
   const int c0 = grp * kN64Chan;
   const int n_chan_here = min(kN64Chan, p.n_chan - c0);
 
@@ -157,7 +168,7 @@ __global__ void __launch_bounds__(kN64Threads, 1) xengine_f32_n64_kernel(const F
         const int j = 4 * tj + ((((b >> 1) ^ sw)) << 1) + (b & 1);
         if (j <= i) {
           const float vim = (j == i) ? 0.f : acc[a][b].y;  // Im of an autocorrelation is exactly 0 (reading R9)
-          if (p.add) red_add_f32x2(rowp + j, acc[a][b].x, vim);
+          if (add) red_add_f32x2(rowp + j, acc[a][b].x, vim);
           else       rowp[j] = make_float2(acc[a][b].x, vim);
         }
       }

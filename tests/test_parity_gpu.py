@@ -268,7 +268,8 @@ def test_set_option_rejects_bad_arguments(pkg):
 # N_I = 64 float path (xengine_f32_n64_kernel: 7-channel groups, time slices with reduce-add): group tails (C not a
 # multiple of 7), slice tails, one slice (plain stores) and many; and the generic 4 x 4 kernel forced on the same shapes.
 @pytest.mark.parametrize("generic", [False, True])
-@pytest.mark.parametrize("C,T", [(1, 1), (7, 16), (8, 17), (15, 100), (150, 33), (23, 700), (300, 260)])
+# (1100, 70) and (1040, 16): more groups than SMs -- whole groups with plain stores plus sliced left-over groups in one launch
+@pytest.mark.parametrize("C,T", [(1, 1), (7, 16), (8, 17), (15, 100), (150, 33), (23, 700), (300, 260), (1100, 70), (1040, 16)])
 def test_cf32_n64_paths_within_tolerance(pkg, generic, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c5"], n_inputs=64, n_chan=C, n_time=T)
     x = w.generate()
