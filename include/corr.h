@@ -171,8 +171,10 @@ enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices force
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
        CORR_OPT_PDL = 6,        /* 0: never launch programmatically inside a stream capture; 1 (default)      */
        CORR_OPT_COLLECT = 7,    /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */
-       CORR_OPT_RESIDENT = 8    /* 0: no resident-A plan (N_I >= 512, T <= 1024: a CTA keeps its A panel of the whole
-                                   integration in shared memory); 1 (default)                                 */ };
+       CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 512, T <= 1024: a CTA keeps its A panel of the whole
+                                   integration in shared memory); 1 (default)                                 */
+       CORR_OPT_MIX = 9         /* 0: N_I <= 64 with more work groups than SMs: every group in the same number of time
+                                   slices; 1 (default): whole groups plus sliced left-over groups                */ };
 int corr_set_option(corr_handle *h, int key, int value);
 
 /*

@@ -15,7 +15,7 @@ from . import build as _build
 CORR_CI8, CORR_CF32, CORR_CI4 = 0, 1, 2
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
 CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
-CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL, CORR_OPT_COLLECT, CORR_OPT_RESIDENT = 1, 2, 3, 4, 5, 6, 7, 8
+CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL, CORR_OPT_COLLECT, CORR_OPT_RESIDENT, CORR_OPT_MIX = 1, 2, 3, 4, 5, 6, 7, 8, 9
 
 # include/corr.h (the product ABI, libcorr.so)
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",

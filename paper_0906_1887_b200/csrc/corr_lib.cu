@@ -78,6 +78,8 @@ struct I8Plan {
   corr::I8Params ip;
   int grid;
   size_t smem;
+  int zero_vis;  // d_vis is zeroed before the launch (items reduce-add: time slices or a mixed plan)
+  int zero_from_chan;  // ... from this channel on (mixed plans: the whole groups in front store plainly)
   int n_batch;  // 0: not planned yet
 };
 
@@ -92,7 +94,7 @@ struct corr_handle {
   int accumulate;
   long long acc_count;      // batches added since corr_set_accumulate(h, 1)
   // plan options (corr_set_option)
-  int opt_diag_plan, opt_pairs, opt_wide, opt_units, opt_f32_generic, opt_pdl, opt_collect, opt_resident;
+  int opt_diag_plan, opt_pairs, opt_wide, opt_units, opt_f32_generic, opt_pdl, opt_collect, opt_resident, opt_mix;
   // CI8 / CI4 plans
   int pair_mode;
   I8Plan plan;        // corr_xengine
@@ -126,6 +128,8 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
   corr::I8Params &ip = out->ip;
   memset(&ip, 0, sizeof ip);
   out->n_batch = n_batch;
+  out->zero_vis = 0;
+  out->zero_from_chan = 0;
   const int N = h->n_inputs, C = h->n_chan, T = h->n_time;
   const int panels_per_chan = h->pair_mode ? 1 : (2 * N + 127) / 128;
   ip.n_time = T; ip.n_inputs = N; ip.n_chan = C; ip.pair_mode = h->pair_mode;
@@ -196,6 +200,27 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     max_load = best_g;
     ip.n_slices = best_s;
     ip.slice_len = best_s == 1 ? T : ((T + best_s - 1) / best_s + 63) / 64 * 64;
+    // Mixed plan: with more groups than CTAs, a x G groups stay whole and only the b left-over groups are cut into
+    // floor(G / b) slices (c2: 192 groups = 148 whole + 44 in thirds: the busiest CTA streams 10000 + 3392 samples
+    // instead of 4 x 3584 with every group in thirds).  Taken when its busiest CTA has less to stream.
+    if (n_batch == 1 && !small && !h->opt_diag_plan && h->opt_mix) {
+      const int a = ip.n_groups / G, b = ip.n_groups % G;
+      if (a >= 1 && b > 0 && G / b >= 2) {
+        int sl = std::min(64, G / b);
+        int len = ((T + sl - 1) / sl + 63) / 64 * 64;
+        sl = (T + len - 1) / len;
+        const long long uniform = ((1LL * ip.n_groups * ip.n_slices + G - 1) / G) * std::min(ip.slice_len, T);
+        const long long mixed = 1LL * a * T + len;
+        if (sl >= 2 && len >= 128 && mixed < uniform) {
+          ip.mix_full = a * G; ip.mix_cut = b; ip.mix_len = len;
+          ip.n_groups = ip.mix_full + b * sl;   // group SLOTS of the walk
+          ip.n_slices = 1; ip.slice_len = T;
+          // only the sliced groups' channels are zeroed: whole groups store (CI8); the 4-bit kernel reduce-adds everywhere
+          out->zero_vis = 1;
+          out->zero_from_chan = h->dtype == CORR_CI8 ? ip.mix_full * ip.gsize * (h->pair_mode ? 2 : 1) : 0;
+        }
+      }
+    }
   } else {
     ip.n_panels = panels_per_chan;
     ip.n_groups = C;
@@ -238,6 +263,7 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     ip.n_slices = 1;
     ip.slice_len = T;
   }
+  if (ip.n_slices > 1) out->zero_vis = 1;
   ip.n_items = ip.n_groups * ip.n_kinds * ip.n_slices * n_batch;
   ip.rot = ip.n_kinds > 1 ? 1 : 0;
   // 32 KB stages: 1 x 256, 2 x 128 or 4 x 64 time rows of 128 B; 48 KB when items fetch 3 panels (3 x 128).  The 4-bit
@@ -427,7 +453,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->probe = 0;
   h->accumulate = 0;
   h->acc_count = 0;
-  h->opt_diag_plan = 0; h->opt_pairs = 1; h->opt_wide = 1; h->opt_units = 0; h->opt_f32_generic = 0; h->opt_pdl = 1; h->opt_collect = 1; h->opt_resident = 1;
+  h->opt_diag_plan = 0; h->opt_pairs = 1; h->opt_wide = 1; h->opt_units = 0; h->opt_f32_generic = 0; h->opt_pdl = 1; h->opt_collect = 1; h->opt_resident = 1; h->opt_mix = 1;
   h->d_items_f32 = nullptr;
   h->d_scratch = nullptr;
   h->d_wide_vis = nullptr;
@@ -494,6 +520,7 @@ int corr_set_option(corr_handle *h, int key, int value) {
     case CORR_OPT_WIDE: h->opt_wide = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_COLLECT: h->opt_collect = value ? 1 : 0; break;
     case CORR_OPT_RESIDENT: h->opt_resident = value ? 1 : 0; break;
+    case CORR_OPT_MIX: h->opt_mix = value ? 1 : 0; break;
     case CORR_OPT_UNITS:
       if (value < 0) return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_UNITS must be >= 0");
       h->opt_units = value;
@@ -827,7 +854,10 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
   ip.accumulate = h->accumulate;
   ip.collect = h->opt_collect;
-  if (ip.n_slices > 1 && !h->accumulate) CUDA_TRY(cudaMemsetAsync(d_vis, 0, h->vis_bytes, st));  // slices accumulate with red.add
+  if (h->plan.zero_vis && !h->accumulate) {  // slices accumulate with red.add
+    const size_t off = static_cast<size_t>(std::min(h->plan.zero_from_chan, h->n_chan)) * h->n_baselines * 8;
+    CUDA_TRY(cudaMemsetAsync(static_cast<char *>(d_vis) + off, 0, h->vis_bytes - off, st));
+  }
   if (h->dtype == CORR_CI4) corr::xengine_i4_kernel<<<grid, corr::kI4Threads, smem, st>>>(*maps, ip);
   else if (ip.pair2) corr::xengine_i8_pair_kernel<<<grid, corr::kI8Threads, smem, st>>>(*maps, ip);
   else {
@@ -885,7 +915,7 @@ int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_v
       if (int rc = get_map(h, d_in[k0 + k], false, &maps)) return rc;
       for (int m = 0; m < 3; ++m) bt.m[k][m] = maps->m[m];
       bt.vis[k] = static_cast<int2 *>(d_vis[k0 + k]);
-      if (ip.n_slices > 1) CUDA_TRY(cudaMemsetAsync(d_vis[k0 + k], 0, h->vis_bytes, st));
+      if (h->plan_batch.zero_vis) CUDA_TRY(cudaMemsetAsync(d_vis[k0 + k], 0, h->vis_bytes, st));
     }
     ip.turned = 0;
     ip.vis = nullptr;

@@ -66,6 +66,7 @@ struct I8Params {
   unsigned long long *diag_stats;  // diagnostics only (probe bit 128): [unit][4] = kernel cycles, MMA waits for loads, MMA waits for TMEM, producer waits for a stage
   int out_shift;     // 8 for 4-bit input (operands are 16 x the samples), else 0
   int accumulate;    // 1: add this integration into d_vis instead of overwriting it
+  int mix_full, mix_cut, mix_len;  // diag plans with more groups than CTAs: whole groups + sliced left-over groups (decode_item)
   int resident;      // 1: CTA pairs keep their A panel of the WHOLE integration in shared memory (T <= 1024) and walk all
                      //    column tiles of a row pair with it; an item is then a unit of two row pairs (xengine_i8_resident.cuh)
   int a_sub;         // resident: 128-row sub-stages of the A region (ceil(T / 128))
@@ -87,6 +88,7 @@ struct I8Item {
   int xa, za;        // TMA coordinates of a separate A panel
   int bk, map;       // time rows per stage and the tensor map (box height) that goes with it
   int chan, I, J0;   // slab: channel, row panel, first column panel; diag: first panel in J0
+  bool sliced;       // mixed plans: this item is a time slice (reduce-add) and not a whole integration (plain stores)
 };
 
 // Tensor maps of one input buffer (box heights 256 / 128 / 64 time rows) and the per-integration arguments of a
@@ -131,12 +133,24 @@ __device__ __forceinline__ bool iter_valid(const I8Params &p, const I8Iter &c) {
 // Decode of a schedule position (all inputs are kernel parameters / uniform counters).
 __device__ __forceinline__ I8Item decode_item(const I8Params &p, const I8Iter &c, int rank = 0) {
   I8Item it;
+  it.sliced = false;
   const int s = c.s, grp = c.grp, k = c.k;
   it.t0 = s * p.slice_len;
   it.t1 = min(p.n_time, it.t0 + p.slice_len);
   const int row = 2 * p.n_inputs;  // bytes per (t, c)
   if (p.diag) {
-    const int panel0 = grp * p.gsize;
+    // mixed plans (more groups than CTAs): the first mix_full group slots are whole integrations, the rest are the
+    // mix_slices time slices of the mix_cut left-over groups, slice-major (the walk itself has n_slices = 1)
+    int g = grp;
+    if (p.mix_cut && g >= p.mix_full) {
+      int u = g - p.mix_full, sl = 0;
+      while (u >= p.mix_cut) { u -= p.mix_cut; ++sl; }
+      g = p.mix_full + u;
+      it.sliced = true;
+      it.t0 = sl * p.mix_len;
+      it.t1 = min(p.n_time, it.t0 + p.mix_len);
+    }
+    const int panel0 = g * p.gsize;
     it.nblk = min(p.gsize, p.n_panels - panel0);
     it.n_load = it.nblk;
     it.a_slot = 0;
@@ -208,6 +222,7 @@ __device__ __forceinline__ ResTile res_tile(const I8Params &p, const I8Iter &c, 
 }
 __device__ __forceinline__ I8Item res_item(const I8Params &p, const I8Iter &c, const ResTile &t, int rank) {
   I8Item it;
+  it.sliced = false;
   it.t0 = 0; it.t1 = p.n_time;
   it.nblk = 2; it.nblk_load = 1; it.jperm = 0; it.n_load = t.diag ? 0 : 1; it.a_slot = 0;
   it.chan = c.grp; it.I = 2 * t.R + rank; it.J0 = t.J0;

@@ -64,17 +64,19 @@ __device__ __forceinline__ EpiTask epi_task(const I8Params &p, const I8Item &it,
 // 4-bit input (operands are 16 x the samples), else 0.  Both are compile-time so that the plain-store path is
 // the bare minimum per value: one SHFL, one IMAD (v + sgn * partner), one conflict-free STS.
 // kPipe: software-pipelined TMEM loads (needs ~50 more registers; off in the 640-thread 4-bit kernel).
-template <bool kAtomic, int kShift, bool kBatch, bool kPipe, bool kResident>
+// kAtomic: 0 = plain stores, 1 = every item reduce-adds (time slices, accumulate mode), 2 = mixed plan: only the items
+// that are time slices reduce-add (I8Item::sliced), whole-integration items store.
+template <int kAtomic, int kShift, bool kBatch, bool kPipe, bool kResident>
 __device__ __forceinline__ void i8_epilogue(const I8Params &p, int2 *const *vis_list, uint32_t tmem_base, uint8_t *stage_buf,
                                             uint64_t *acc_full, uint64_t *acc_empty, int n_rounds, int ew,
                                             int hsel, int lane, int rank, bool pair, int probe) {
   const int part = lane & 1;  // 0: row 2i (Re row of input i), 1: row 2i+1 (Im row)
   const int rl = lane >> 1;   // which of the warp's 16 inputs this lane pair holds
-  constexpr bool atomic = kAtomic;
   const int sgn = part ? -1 : 1;  // Re = G[2i][2j] + G[2i+1][2j+1], Im = G[2i+1][2j] - G[2i][2j+1]
   // staging row stride: 272 B keeps rows 16-byte aligned for the bulk reduce-add; 264 B (66 words) makes the
   // 4-byte staging writes of the 32 lanes hit 32 different banks on the plain-store path
   constexpr int kRowB = kAtomic ? kEpiRowBytes : kEpiRowBytesPlain;
+  bool any_atomic = false;
   int *st_w = reinterpret_cast<int *>(stage_buf) + rl * (kRowB / 4) + part;
   uint32_t ring = 0;
   I8Iter cur = iter_init(p);
@@ -84,6 +86,8 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, int2 *const *vis_
     for (int sub = 0; sub < n_sub; ++sub) {
     const I8Item it = (kResident && p.resident) ? res_item(p, cur, res_tile(p, cur, sub), rank) : decode_item(p, cur, rank);
     int2 *const vis = kBatch ? vis_list[cur.bi] : p.vis;  // output of this item's integration
+    const bool atomic = kAtomic == 1 || (kAtomic == 2 && it.sliced);
+    any_atomic = any_atomic || atomic;
     const int n_chunks = (it.nblk + 1) >> 1;
     for (int q = 0; q < n_chunks; ++q) {
       const uint32_t e = ring + q;
@@ -122,7 +126,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, int2 *const *vis_
         const int par = atomic ? static_cast<int>((static_cast<long long>(tk.chan_w) * p.n_baselines +
                                                     i_row * (i_row + 1) / 2 + tk.j0) & 1) : 0;
         int *st_row = st_w + par * 2;
-        if (atomic && lane < 16) bulk_wait_read_all();  // earlier bulk reduces have read the staging buffer
+        if (kAtomic && lane < 16) bulk_wait_read_all();  // earlier bulk reduces have read the staging buffer
         __syncwarp();  // the previous half block has been read out of the staging buffer
         tmem_ld_wait_regs(v0);
         tmem_ld_wait_regs(v1);
@@ -210,7 +214,7 @@ __device__ __forceinline__ void i8_epilogue(const I8Params &p, int2 *const *vis_
     ring += n_chunks;
     }
   }
-  if (atomic && lane < 16) bulk_wait_all();  // all reduce-adds performed before the CTA retires
+  if (kAtomic && any_atomic && lane < 16) bulk_wait_all();  // all reduce-adds performed before the CTA retires
 }
 
 }  // namespace corr

@@ -342,12 +342,15 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
     const int ew = warp & 3;         // TMEM lanes 32*ew .. 32*ew+31 (a warp may only touch its own quadrant)
     const int hsel = warp >> 2;        // which half (64 TMEM columns) of every block this warp folds
     constexpr int kShift = kPacked ? 8 : 0;
-    if (p.n_slices > 1 || p.accumulate)
-      i8_epilogue<true, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
-                                        acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+    if (p.n_slices > 1 || p.accumulate || ((kPair || kBatch || kPacked) && p.mix_cut))
+      i8_epilogue<1, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                                      acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+    else if (!kPair && !kBatch && !kPacked && p.mix_cut)  // mixed plan: whole groups store, their sliced neighbours reduce-add
+      i8_epilogue<2, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                                      acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
     else
-      i8_epilogue<false, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
-                                         acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
+      i8_epilogue<0, kShift, kBatch, !kPacked, kPair>(p, vis_list, tmem_base, epi_stage + warp * kEpiWarpBytes,
+                                                      acc_full, acc_empty, n_rounds, ew, hsel, lane, rank, kPair, probe);
   }
 
   tc_fence_before();

@@ -27,7 +27,9 @@ def run_ci4(x_packed):
 
 
 SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 33), (64, 1, 257), (64, 200, 40), (32, 4, 100), (32, 3, 70),
-          (32, 301, 33), (96, 2, 64), (128, 2, 300), (256, 2, 130), (320, 1, 64), (1024, 1, 96)]
+          (32, 301, 33), (96, 2, 64), (128, 2, 300), (256, 2, 130), (320, 1, 64), (1024, 1, 96),
+          # > 64 MB with more panel groups than SMs: the mixed whole / sliced plan (every item reduce-adds in this kernel)
+          (64, 1300, 900)]
 
 
 @pytest.mark.parametrize("N,C,T", SHAPES)

@@ -256,6 +256,16 @@ def test_ci8_diag_plans_bit_exact(pkg, plan, N, C, T):
     assert np.array_equal(out, oracle.xengine_ci8(x, threads=_threads()))
 
 
+# Mixed plans (inputs > 64 MB with more panel groups than SMs): a x 148 groups run as whole integrations with plain
+# stores, the left-over groups as time slices that reduce-add into their zeroed channels -- in ONE launch.
+@pytest.mark.parametrize("N,C,T,mix", [(64, 700, 800, 1), (32, 1300, 900, 1), (64, 700, 800, 0)])
+def test_ci8_mixed_whole_and_sliced_groups_bit_exact(pkg, N, C, T, mix):
+    w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    out = run_ci8(pkg, x, options=[(pkg.CORR_OPT_MIX, mix)])
+    assert np.array_equal(out, oracle.xengine_ci8(x, threads=_threads()))
+
+
 def test_set_option_rejects_bad_arguments(pkg):
     h = pkg.corr_create(64, 2, 100, "ci8")
     for key, value in [(99, 1), (pkg.CORR_OPT_DIAG_PLAN, 256 * 3 + 1), (pkg.CORR_OPT_DIAG_PLAN, 256 * 4 + 65), (pkg.CORR_OPT_UNITS, -1)]:
