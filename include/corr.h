@@ -169,7 +169,8 @@ enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices force
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
        CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
-       CORR_OPT_PDL = 6,        /* 0: never launch programmatically inside a stream capture; 1 (default)      */
+       CORR_OPT_PDL = 6,        /* programmatic dependent launch of the single-CTA int8 kernel: 0 never; 1 (default) inside a
+                                   stream capture and for inputs above 64 MB; 2 always                           */
        CORR_OPT_COLLECT = 7,    /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */
        CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 512, T <= 1024: a CTA keeps its A panel of the whole
                                    integration in shared memory); 1 (default)                                 */

@@ -526,7 +526,7 @@ int corr_set_option(corr_handle *h, int key, int value) {
       h->opt_units = value;
       break;
     case CORR_OPT_F32_GENERIC: h->opt_f32_generic = value ? 1 : 0; break;
-    case CORR_OPT_PDL: h->opt_pdl = value ? 1 : 0; break;
+    case CORR_OPT_PDL: h->opt_pdl = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     default: return fail(CORR_EINVAL, "corr_set_option: unknown key %d", key);
   }
   return replan(h);
@@ -863,11 +863,12 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   else {
     // programmatic dependent launch: the kernel may start while the preceding kernel of the stream drains (it waits with
     // griddepcontrol.wait before its first global-memory access); worth ~1 us per call on launch-bound inputs (c1: 7.5 ->
-    // 6.2 us in a replayed graph).  Only while the stream is being captured into a CUDA graph: launched call by call
-    // the attribute costs more host time per launch than it saves on the device.
+    // 6.2 us in a replayed graph).  For small inputs only while the stream is being captured into a CUDA graph: launched
+    // call by call the attribute costs more host time per launch than it saves on the device; inputs above 64 MB run long
+    // enough to hide that (c2: 160.7 -> 158.6 us call by call).
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (h->opt_pdl && cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cap = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
-    if (h->opt_pdl && cap == cudaStreamCaptureStatusActive) {
+    if (h->opt_pdl == 2 || (h->opt_pdl && (cap == cudaStreamCaptureStatusActive || h->in_bytes > (64u << 20)))) {
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3(grid); cfg.blockDim = dim3(corr::kI8Threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
       cudaLaunchAttribute attr[1];
