@@ -222,3 +222,54 @@ def test_ci4_wide_rows_keep_a_deep_ring(pkg):
         torch.cuda.synchronize()
         assert np.array_equal(v.cpu().numpy(), oracle.xengine_ci4(x4, threads=_threads())), (N, C, T)
         pkg.corr_destroy(h)
+
+
+def test_batch_of_one_and_replanning_between_sizes(pkg):
+    """n = 1 is an ordinary call; a handle re-plans when the batch size changes (3 -> 64 -> 3) and stays usable for
+    single calls in between; options set after the first use re-plan as well."""
+    N, C, T = 32, 10, 90
+    w = corrgen.scaled(corrgen.CONFIGS["c1"], n_inputs=N, n_chan=C, n_time=T)
+    xs = [w.generate(integration=k) for k in range(64)]
+    refs = [oracle.xengine_ci8(x, threads=_threads()) for x in xs[:4]] + [None] * 60
+    d_in = [torch.from_numpy(x).cuda() for x in xs]
+    h = pkg.corr_create(N, C, T, "ci8")
+    for n in (1, 3, 64, 3):
+        outs = [h.empty_vis().fill_(POISON) for _ in range(n)]
+        pkg.corr_xengine_batch(h, d_in[:n], outs)
+        torch.cuda.synchronize()
+        for k in range(min(n, 4)):
+            assert np.array_equal(outs[k].cpu().numpy(), refs[k]), (n, k)
+        if n == 64:
+            k = 63
+            assert np.array_equal(outs[k].cpu().numpy(), oracle.xengine_ci8(xs[k], threads=_threads()))
+        single = pkg.corr_xengine(h, d_in[2])
+        torch.cuda.synchronize()
+        assert np.array_equal(single.cpu().numpy(), refs[2])
+    h.set_option(pkg.CORR_OPT_DIAG_PLAN, 256 * 2 + 2)
+    outs = pkg.corr_xengine_batch(h, d_in[:3])
+    torch.cuda.synchronize()
+    for k in range(3):
+        assert np.array_equal(outs[k].cpu().numpy(), refs[k])
+    pkg.corr_destroy(h)
+
+
+def test_window_with_accumulate_and_wide_accumulators(pkg):
+    """A channel-window handle in accumulate mode and with corr_accumulate_wide: batches of the window add up."""
+    N, C, T = 64, 9, 70
+    w = corrgen.scaled(corrgen.CONFIGS["c2"], n_inputs=N, n_chan=C, n_time=T)
+    xs = [w.generate(integration=k) for k in range(3)]
+    want = oracle.xengine_ci8_wide(np.concatenate(xs, axis=0), 2, 7, threads=_threads())
+    h = pkg.corr_create(N, 5, T, "ci8")
+    h.set_chan_window(C, 2)
+    h.set_accumulate(True)
+    vis = h.empty_vis().zero_()
+    acc = h.empty_acc()
+    for x in xs:
+        d = torch.from_numpy(x).cuda()
+        pkg.corr_xengine(h, d, vis)
+        h.accumulate_wide(d, acc)
+    torch.cuda.synchronize()
+    assert h.accumulate_count == 3
+    assert np.array_equal(vis.cpu().numpy().astype(np.int64), want)
+    assert np.array_equal(acc.cpu().numpy(), want)
+    pkg.corr_destroy(h)
