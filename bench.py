@@ -550,6 +550,41 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     return out
 
 
+def curve_entry(pkg, torch, peaks, steps=10, warmup=3):
+    """The metric's own axis: useful CMAC/s versus N_I at a fixed input volume (~0.5 GB of int8 samples, T = 2000, c4's
+    sample recipe), with each point's roofline fraction (HBM or 2 x measured bf16, burst and sustained)."""
+    import corrgen
+    out = []
+    T = 2000
+    for n in (32, 64, 128, 256, 512, 1024, 2048, 4096):
+        c = max(1, (512 << 20) // (T * 2 * n))
+        w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=n, n_chan=c, n_time=T)
+        x = torch.from_numpy(w.generate()).cuda()
+        h = pkg.corr_create(n, c, T, "ci8")
+        vis = h.empty_vis()
+        stream = torch.cuda.current_stream()
+        for _ in range(warmup):
+            h.xengine(x, vis, stream)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ev[0].record(stream)
+        for k in range(steps):
+            h.xengine(x, vis, stream)
+            ev[k + 1].record(stream)
+        torch.cuda.synchronize()
+        per = sorted(ev[k].elapsed_time(ev[k + 1]) * 1e-3 for k in range(steps))
+        sec = per[len(per) // 2]
+        t_a = w.in_bytes / (peaks["hbm_gbs"] * 1e9)
+        t_burst = 8.0 * w.cmacs / (2.0 * peaks["bf16_tflops"] * 1e12)
+        t_sus = 8.0 * w.cmacs / (2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * 1e12)
+        out.append({"n_inputs": n, "n_chan": c, "n_time": T, "ms": sec * 1e3, "value": w.cmacs / sec, "unit": UNIT,
+                    "bound": "hbm" if t_a >= t_burst else "tensor", "frac_burst": max(t_a, t_burst) / sec,
+                    "frac_sustained": max(t_a, t_sus) / sec})
+        h.destroy()
+        del x, vis
+        torch.cuda.empty_cache()
+    return out
+
+
 def packed_entry(pkg, torch, peaks, steps=50, warmup=5, n_inputs=None, n_chan=None, n_time=None):
     """c2 in the paper's 1-byte mode (4+4-bit samples): half the input bytes.
     With n_inputs / n_chan / n_time: the same recipe at another shape (the slab plans of the 4-bit kernel)."""
@@ -800,6 +835,10 @@ def main():
             sweep["c5_fstage"] = fstage_entry(pkg, torch, peaks)
         except Exception as e:
             sweep["c5_fstage"] = {"error": str(e)[:200]}
+        try:
+            sweep["vs_n_inputs"] = curve_entry(pkg, torch, peaks)
+        except Exception as e:
+            sweep["vs_n_inputs"] = {"error": str(e)[:200]}
         line["by_config"] = sweep
     print(json.dumps(line), flush=True)
     if dist is not None:

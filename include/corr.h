@@ -164,7 +164,8 @@ int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
  * the handle; the defaults are what corr_create chose.  CORR_EINVAL for an unknown key or a value out of range.
  */
 enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
-                                   panels per work item and `slices` (1..64) time slices; 0 = automatic       */
+                                   panels per work item and `slices` (1..64) time slices (slices = 0: only the
+                                   group width is forced); 0 = automatic                                     */
        CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
        CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */

@@ -163,11 +163,9 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
         const double t = rounds * g / rate[g];
         if (t < best_t * 0.999) { best_t = t; best_g = g; }
       }
-    } else {
-      for (int g = 4; g >= (small ? 1 : 4); g >>= 1) {
+    } else if (small) {
+      for (int g = 4; g >= 1; g >>= 1) {
         const int base = (ip.n_panels + g - 1) / g;
-        int cand_s = 1;
-        double cand_eff = 0.0;
         for (int s = 1; s <= 64; ++s) {
           int len = ((T + s - 1) / s + 63) / 64 * 64;
           if (len < 128 && s > 1) break;
@@ -175,24 +173,46 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
           if (s_eff != s) continue;
           const long long n = 1LL * base * s;
           const long long rounds = (n + G - 1) / G;
-          // load of the busiest CTA in units of samples vs the mean
-          const double eff = (1.0 * base * T / G) / (1.0 * rounds * len);
-          if (small) {
-            // modelled time: rounds x (item bytes at ~80 GB/s per SM) + the fixed cost of a sliced launch
-            const double t = 1e-9 * rounds * (1.0 * g * 128 * std::min(len, T)) / 80.0 + (s > 1 ? 4e-6 : 0.0);
-            if (t < best_t - 1e-7) { best_t = t; best_g = g; best_s = s; }
-          } else {
-            if (eff > cand_eff + 0.02) { cand_eff = eff; cand_s = s; }
-            if (cand_eff >= 0.95) break;
-          }
+          // modelled time: rounds x (item bytes at ~80 GB/s per SM) + the fixed cost of a sliced launch
+          const double t = 1e-9 * rounds * (1.0 * g * 128 * std::min(len, T)) / 80.0 + (s > 1 ? 4e-6 : 0.0);
+          if (t < best_t - 1e-7) { best_t = t; best_g = g; best_s = s; }
         }
-        if (!small) best_s = cand_s;
       }
     }
-    if (h->opt_diag_plan) {  // corr_set_option(CORR_OPT_DIAG_PLAN): 256 * gsize + slices
+    int mix_sl = 0, mix_len = 0;  // > 0: mixed plan (whole groups + the left-over groups in mix_sl slices of mix_len)
+    if (n_batch == 1 && !small) {
+      // Large inputs stream from HBM: model the busiest CTA's time for every (group width g, plan) and take the least.
+      //   per sample a CTA streams g x 128 B at its share of the HBM rate (narrower runs fetch a little slower);
+      //   per item it pays the part of the epilogue the next item's loads cannot hide: all of it with g = 4 (the four
+      //   accumulators fill TMEM), little with g = 2 (double-buffered), more when the item reduce-adds;
+      //   uniform plan: every group in s slices; mixed plan: a x G whole groups (plain stores, no zeroing) + the b
+      //   left-over groups in s slices (c2: 148 whole + 44 groups in thirds).
+      const double bw = 6.5e12 / G;
+      const int g_lo = (h->opt_diag_plan >> 8) ? (h->opt_diag_plan >> 8) : 2, g_hi = (h->opt_diag_plan >> 8) ? (h->opt_diag_plan >> 8) : 4;
+      for (int g = g_hi; g >= g_lo; g >>= 1) {
+        if (g == 1 && !(h->opt_diag_plan >> 8)) continue;
+        const double ts = g * 128.0 / (bw * (g == 4 ? 1.0 : g == 2 ? 0.92 : 0.70));
+        const double epi = g == 4 ? 4.0e-6 : 0.5e-6, epi_add = g == 4 ? 5.0e-6 : 1.0e-6;
+        const int groups = (ip.n_panels + g - 1) / g;
+        for (int sl = 1; sl <= 64; ++sl) {
+          const int len = sl == 1 ? T : ((T + sl - 1) / sl + 63) / 64 * 64;
+          if (sl > 1 && (len < 128 || (T + len - 1) / len != sl)) { if (len < 128) break; continue; }
+          const long long rounds = (1LL * groups * sl + G - 1) / G;
+          const double t = rounds * (std::min(len, T) * ts + (sl > 1 ? epi_add : epi)) + (sl > 1 ? 3e-6 : 0.0);
+          if (t < best_t * 0.98) { best_t = t; best_g = g; best_s = sl; mix_sl = 0; }
+          const int a = groups / G, b = groups % G;
+          if (sl > 1 && a >= 1 && b > 0 && h->opt_mix && !(h->opt_diag_plan & 255)) {
+            const long long r2 = (1LL * b * sl + G - 1) / G;
+            const double tm = a * (T * ts + epi) + r2 * (len * ts + epi_add) + 2e-6;
+            if (tm < best_t * 0.98) { best_t = tm; best_g = g; best_s = 1; mix_sl = sl; mix_len = len; }
+          }
+        }
+      }
+    }
+    if (h->opt_diag_plan & 255) {  // corr_set_option(CORR_OPT_DIAG_PLAN): 256 * gsize + slices forces a uniform plan
       const int g = h->opt_diag_plan >> 8, sl = h->opt_diag_plan & 255;
       const int len = ((T + sl - 1) / sl + 63) / 64 * 64;
-      if (sl == 1 || (len >= 128 && (T + len - 1) / len == sl)) { best_g = g; best_s = sl; }
+      if (sl == 1 || (len >= 128 && (T + len - 1) / len == sl)) { best_g = g; best_s = sl; mix_sl = 0; }
     }
     ip.gsize = best_g;
     ip.n_groups = (ip.n_panels + best_g - 1) / best_g;
@@ -200,26 +220,12 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     max_load = best_g;
     ip.n_slices = best_s;
     ip.slice_len = best_s == 1 ? T : ((T + best_s - 1) / best_s + 63) / 64 * 64;
-    // Mixed plan: with more groups than CTAs, a x G groups stay whole and only the b left-over groups are cut into
-    // floor(G / b) slices (c2: 192 groups = 148 whole + 44 in thirds: the busiest CTA streams 10000 + 3392 samples
-    // instead of 4 x 3584 with every group in thirds).  Taken when its busiest CTA has less to stream.
-    if (n_batch == 1 && !small && !h->opt_diag_plan && h->opt_mix) {
-      const int a = ip.n_groups / G, b = ip.n_groups % G;
-      if (a >= 1 && b > 0 && G / b >= 2) {
-        int sl = std::min(64, G / b);
-        int len = ((T + sl - 1) / sl + 63) / 64 * 64;
-        sl = (T + len - 1) / len;
-        const long long uniform = ((1LL * ip.n_groups * ip.n_slices + G - 1) / G) * std::min(ip.slice_len, T);
-        const long long mixed = 1LL * a * T + len;
-        if (sl >= 2 && len >= 128 && mixed < uniform) {
-          ip.mix_full = a * G; ip.mix_cut = b; ip.mix_len = len;
-          ip.n_groups = ip.mix_full + b * sl;   // group SLOTS of the walk
-          ip.n_slices = 1; ip.slice_len = T;
-          // only the sliced groups' channels are zeroed: whole groups store (CI8); the 4-bit kernel reduce-adds everywhere
-          out->zero_vis = 1;
-          out->zero_from_chan = h->dtype == CORR_CI8 ? ip.mix_full * ip.gsize * (h->pair_mode ? 2 : 1) : 0;
-        }
-      }
+    if (mix_sl > 1) {
+      ip.mix_full = (ip.n_groups / G) * G; ip.mix_cut = ip.n_groups % G; ip.mix_len = mix_len;
+      ip.n_groups = ip.mix_full + ip.mix_cut * mix_sl;   // group SLOTS of the walk
+      // only the sliced groups' channels are zeroed: whole groups store (CI8); the 4-bit kernel reduce-adds everywhere
+      out->zero_vis = 1;
+      out->zero_from_chan = h->dtype == CORR_CI8 ? ip.mix_full * ip.gsize * (h->pair_mode ? 2 : 1) : 0;
     }
   } else {
     ip.n_panels = panels_per_chan;
@@ -511,7 +517,7 @@ int corr_set_option(corr_handle *h, int key, int value) {
   switch (key) {
     case CORR_OPT_DIAG_PLAN: {
       const int g = value >> 8, sl = value & 255;
-      if (value != 0 && !((g == 1 || g == 2 || g == 4) && sl >= 1 && sl <= 64))
+      if (value != 0 && !((g == 1 || g == 2 || g == 4) && sl >= 0 && sl <= 64))
         return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_DIAG_PLAN wants 256 * gsize (1, 2, 4) + slices (1..64), got %d", value);
       h->opt_diag_plan = value;
       break;
