@@ -233,7 +233,10 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     int k = 0;
     // CTA pairs (cta_group::2) from N_I = 512 up; already from N_I = 256 when the integration is long
     // enough (T >= 2048) for 512-wide tiles, whose epilogue cannot overlap the next tile's MMAs
-    const bool long_ok = (T >= 2048 || h->opt_wide == 2) && panels_per_chan >= 4;
+    // ... and only up to N_I = 448: from 8 panels per channel on, 256-wide tiles find their panels in L2 and hide every
+    // epilogue, which beats the 512-wide tiles' leaner operand traffic (N_I = 512 / 1024 / 2048 at T = 4000: 287 -> 238,
+    // 480 -> 406, 819 -> 726 us)
+    const bool long_ok = ((T >= 2048 && panels_per_chan < 8) || h->opt_wide == 2) && panels_per_chan >= 4;
     const bool wide_ok = long_ok && h->opt_wide;
     if (use_pairs && panels_per_chan >= 8 && !long_ok && T <= 128 * corr::kResMaxSub && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
       // resident-A plan (xengine_i8_resident.cuh): the A panel of the whole integration stays in shared memory; an item

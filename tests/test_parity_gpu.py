@@ -108,11 +108,19 @@ def test_ci8_pair_tiles_without_the_resident_plan(pkg, N, C, T):
     assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_RESIDENT, 0)]), oracle.xengine_ci8(x, threads=_threads()))
 
 
-@pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (512, 1, 2081)])
+@pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (384, 1, 2081)])
 def test_ci8_wide_pair_tiles_without_collector_reuse(pkg, N, C, T):
     w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
     x = w.generate()
     assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_COLLECT, 0)]), oracle.xengine_ci8(x, threads=_threads()))
+
+
+@pytest.mark.parametrize("N,C,T", [(512, 1, 2081), (640, 1, 1030)])
+def test_ci8_wide_pair_tiles_forced_for_many_panels(pkg, N, C, T):
+    """CORR_OPT_WIDE = 2: 512-wide tiles also from N_I = 512 up and for short integrations (by default 256-wide there)."""
+    w = corrgen.scaled(corrgen.CONFIGS["c4"], n_inputs=N, n_chan=C, n_time=T)
+    x = w.generate()
+    assert np.array_equal(run_ci8(pkg, x, options=[(pkg.CORR_OPT_WIDE, 2)]), oracle.xengine_ci8(x, threads=_threads()))
 
 
 @pytest.mark.parametrize("N,C,T", [(256, 2, 2100), (512, 1, 2081)])
