@@ -142,7 +142,7 @@ int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out,
  *   d_vis : HOST array of n device pointers, each as corr_xengine's d_vis (distinct buffers)
  *   n     : >= 1; more than 64 integrations are issued as several launches of <= 64
  * Same result as n corr_xengine calls (bit-exact for CI8).  The single-launch path covers CORR_CI8 shapes
- * that run on single CTAs (N_I <= 64, and 128 <= N_I < 512 unless the integration is long); every other
+ * that run on single CTAs (N_I <= 128, and 256 <= N_I < 512 with 1024 < T < 2048); every other
  * case (CTA-pair plans, CORR_CI4, CORR_CF32, the standalone corner turn, accumulate mode) falls back to n
  * ordinary calls on `stream`.  Returns as corr_xengine.
  */
@@ -166,14 +166,15 @@ int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
 enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
                                    panels per work item and `slices` (1..64) time slices (slices = 0: only the
                                    group width is forced); 0 = automatic                                     */
-       CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
+       CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned;
+                                   2: CTA pairs from N_I = 128 up (experiments)                                 */
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
        CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
        CORR_OPT_PDL = 6,        /* programmatic dependent launch of the single-CTA int8 kernel: 0 never; 1 (default) inside a
                                    stream capture and for inputs above 64 MB; 2 always                           */
        CORR_OPT_COLLECT = 7,    /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */
-       CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 512, T <= 1024: a CTA keeps its A panel of the whole
+       CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 256, T <= 1024: a CTA keeps its A panel of the whole
                                    integration in shared memory); 1 (default)                                 */
        CORR_OPT_MIX = 9         /* 0: N_I <= 64 with more work groups than SMs: every group in the same number of time
                                    slices; 1 (default): whole groups plus sliced left-over groups                */ };

@@ -238,7 +238,10 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     // 480 -> 406, 819 -> 726 us)
     const bool long_ok = ((T >= 2048 && panels_per_chan < 8) || h->opt_wide == 2) && panels_per_chan >= 4;
     const bool wide_ok = long_ok && h->opt_wide;
-    if (use_pairs && panels_per_chan >= 8 && !long_ok && T <= 128 * corr::kResMaxSub && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
+    const int min_pair_panels = h->opt_pairs == 2 ? 2 : 8;  // CORR_OPT_PAIRS = 2 (experiments): CTA pairs from N_I = 128 up
+    // the resident-A plan already from N_I = 256 (N_I = 256 / 384 at T = 1000: 185 -> 175, 252 -> 217 us against single-CTA slabs)
+    const int min_res_panels = h->opt_pairs == 2 ? 2 : 4;
+    if (use_pairs && panels_per_chan >= min_res_panels && !long_ok && T <= 128 * corr::kResMaxSub && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
       // resident-A plan (xengine_i8_resident.cuh): the A panel of the whole integration stays in shared memory; an item
       // is a unit of two row pairs (pp - 1 - u and u: pp + 1 tiles in every unit)
       ip.pair2 = 1;
@@ -247,7 +250,7 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
       const int pp = (panels_per_chan + 1) / 2;
       for (int u = 0; u < (pp + 1) / 2; ++u) ip.kinds[k++] = static_cast<unsigned short>(u);
       max_load = 1;
-    } else if (use_pairs && (panels_per_chan >= 8 || long_ok)) {
+    } else if (use_pairs && (panels_per_chan >= min_pair_panels || long_ok)) {
       ip.pair2 = 1;
       const int pp = (panels_per_chan + 1) / 2;
       max_load = 2;
@@ -525,7 +528,7 @@ int corr_set_option(corr_handle *h, int key, int value) {
       h->opt_diag_plan = value;
       break;
     }
-    case CORR_OPT_PAIRS: h->opt_pairs = value ? 1 : 0; break;
+    case CORR_OPT_PAIRS: h->opt_pairs = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_WIDE: h->opt_wide = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_COLLECT: h->opt_collect = value ? 1 : 0; break;
     case CORR_OPT_RESIDENT: h->opt_resident = value ? 1 : 0; break;
