@@ -126,6 +126,38 @@ int corr_normalize_wide(corr_handle *h, const void *d_acc, double count, void *d
 size_t corr_acc_bytes(const corr_handle *h); /* 2 * corr_vis_bytes */
 
 /*
+ * corr_accumulate_wide_static -- corr_accumulate_wide for callers that must not allocate device memory.
+ *
+ * Who needs it: a correlator's real-time loop, or a plug-in living inside a host application that has already
+ * handed all of the GPU's memory to its own pool.  cudaMalloc / cudaFree synchronise the whole device (every
+ * stream stalls while they run, which a loop with a sample-rate deadline cannot afford), they can fail once another
+ * owner holds the memory, and some hosts simply forbid them after start-up.  corr_accumulate_wide allocates its
+ * batch buffer (corr_vis_bytes) on the handle's first call; this entry point never does.  The batch of
+ * PAPER.md:125 / :166 is computed into a buffer that is part of the library image itself: a fixed device array
+ * of CORR_STATIC_BATCH_BYTES, which every GPU that loads the library carries from load to process exit, used or
+ * not.  The batch is then folded, acc[k] += vis[k], into the caller's d_acc exactly as corr_accumulate_wide does
+ * (same arguments, same results bit for bit).  With a CORR_CI8 / CORR_CI4 handle the whole sequence corr_create ->
+ * corr_accumulate_wide_static -> corr_normalize_wide -> corr_destroy makes no device allocation at all (a
+ * CORR_CF32 handle allocates its work-item table in corr_create, none afterwards).
+ *
+ * Limits and rules:
+ *   - corr_vis_bytes(h) <= CORR_STATIC_BATCH_BYTES, else CORR_EUNSUPPORTED and nothing is enqueued (of the paper-
+ *     shaped configurations c1, c2 and c5-sized cubes up to 16 MiB fit; N_I = 256 x 512 channels does not);
+ *   - no cudaMalloc, cudaFree or allocating library routine is called, on any call;
+ *   - the FIRST call on each device looks up the array's device address (one query, with that device current,
+ *     which may make the CUDA runtime finish loading the library's module): make that call during set-up,
+ *     before any stream capture and before the deadline-bound loop starts; later calls on that device only launch;
+ *   - the array is shared by every handle, stream and thread of the process on that GPU and keeps whatever the
+ *     last call left in it.  Nothing in it has to start at zero -- each call overwrites (or, for time-sliced plans,
+ *     clears on `stream` and then fills) the corr_vis_bytes(h) it uses before folding them -- but two calls whose
+ *     GPU work can overlap (different streams without an event between them, or two host threads) RACE on it and
+ *     corrupt both accumulations.  Keep all calls on one device stream-ordered.
+ * Asynchronous on `stream`.  Returns CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED or CORR_ECUDA (never CORR_EALLOC).
+ */
+#define CORR_STATIC_BATCH_BYTES (16u << 20)
+int corr_accumulate_wide_static(corr_handle *h, const void *d_in, void *d_acc, void *stream);
+
+/*
  * corr_normalize -- read-out (the accumulators are "divided by the number of times they were
  * updated"): d_out[c][b] = d_vis[c][b] / count as (float re, float im); d_vis holds int32 pairs (CI8, CI4)
  * or float pairs (CF32).  d_out has corr_vis_bytes(h) bytes, 16-byte aligned, may not alias d_vis unless the

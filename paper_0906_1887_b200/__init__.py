@@ -15,13 +15,14 @@ from . import build as _build
 CORR_CI8, CORR_CF32, CORR_CI4 = 0, 1, 2
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_EALLOC, CORR_ECUDA, CORR_EARCH = range(6)
 CORR_TURN_FUSED, CORR_TURN_STANDALONE = 0, 1
+CORR_STATIC_BATCH_BYTES = 16 << 20   # include/corr.h: capacity of corr_accumulate_wide_static's built-in batch buffer
 CORR_OPT_DIAG_PLAN, CORR_OPT_PAIRS, CORR_OPT_WIDE, CORR_OPT_UNITS, CORR_OPT_F32_GENERIC, CORR_OPT_PDL, CORR_OPT_COLLECT, CORR_OPT_RESIDENT, CORR_OPT_MIX = 1, 2, 3, 4, 5, 6, 7, 8, 9
 
 # include/corr.h (the product ABI, libcorr.so)
 EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "corr_last_status",
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
            "corr_corner_turn", "corr_stream_run", "corr_set_accumulate", "corr_accumulate_count", "corr_normalize",
-           "corr_accumulate_wide", "corr_normalize_wide", "corr_acc_bytes", "corr_xengine_batch", "corr_set_chan_window",
+           "corr_accumulate_wide", "corr_accumulate_wide_static", "corr_normalize_wide", "corr_acc_bytes", "corr_xengine_batch", "corr_set_chan_window",
            "corr_set_option",
            "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx", "corr_fstage_set_input")
 # include/corr_diag.h (diagnostics, libcorr_diag.so only)
@@ -65,6 +66,7 @@ def _bind(path, diag):
     L.corr_normalize_wide.restype = ci
     L.corr_normalize_wide.argtypes = [vp, vp, ctypes.c_double, vp, vp]
     L.corr_accumulate_wide.restype, L.corr_accumulate_wide.argtypes = ci, [vp, vp, vp, vp]
+    L.corr_accumulate_wide_static.restype, L.corr_accumulate_wide_static.argtypes = ci, [vp, vp, vp, vp]
     L.corr_acc_bytes.restype, L.corr_acc_bytes.argtypes = ctypes.c_size_t, [vp]
     L.corr_xengine_batch.restype = ci
     L.corr_xengine_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ci, vp]
@@ -203,6 +205,18 @@ class Correlator:
         if not d_acc.is_cuda or not d_acc.is_contiguous() or d_acc.numel() * d_acc.element_size() != 2 * self.vis_bytes:
             raise ValueError(f"d_acc must be a contiguous CUDA tensor of {2 * self.vis_bytes} bytes")
         if lib().corr_accumulate_wide(self._h, d_in.data_ptr(), d_acc.data_ptr(), _stream_ptr(stream)) != CORR_OK:
+            _raise()
+        return d_acc
+
+    def accumulate_wide_static(self, d_in, d_acc, stream=None):
+        """corr_accumulate_wide_static: accumulate_wide() for code that must not allocate device memory (a real-time
+        loop that cannot take cudaMalloc's device-wide stall, a host application whose pool owns all of the GPU).  The
+        batch is staged in a fixed array inside the library (CORR_STATIC_BATCH_BYTES; larger vis_bytes raise CorrError),
+        shared by every handle on the GPU: keep calls stream-ordered, and make the first call during set-up."""
+        self._check_in(d_in)
+        if not d_acc.is_cuda or not d_acc.is_contiguous() or d_acc.numel() * d_acc.element_size() != 2 * self.vis_bytes:
+            raise ValueError(f"d_acc must be a contiguous CUDA tensor of {2 * self.vis_bytes} bytes")
+        if lib().corr_accumulate_wide_static(self._h, d_in.data_ptr(), d_acc.data_ptr(), _stream_ptr(stream)) != CORR_OK:
             _raise()
         return d_acc
 

@@ -16,6 +16,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <cmath>
+#include <mutex>
 #include <queue>
 #include <vector>
 
@@ -28,6 +29,32 @@
 #include "xengine_f32.cuh"
 #include "xengine_f32_n64.cuh"
 #include "xengine_i8.cuh"
+
+// Batch buffer of corr_accumulate_wide_static (include/corr.h): device memory that belongs to the library image, so
+// that the entry point has nothing to allocate.  Host code may NOT use this name as a pointer -- on the host it is only
+// a stand-in for the symbol; static_batch_ptr() below asks the runtime for the array's address on the current device.
+static __device__ __align__(256) unsigned char g_static_batch[CORR_STATIC_BATCH_BYTES];
+
+// corr::fold_wide_kernel (readout.cuh) with the batch read from g_static_batch: device code names the array directly.
+// acc[k] += batch[k], int32 -> int64 or float -> double, n scalars (a multiple of 4), 16-byte vectors, grid-stride.
+__global__ void __launch_bounds__(256) fold_wide_static_kernel(void *acc, long long n, int is_int) {
+  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  for (long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; k < n / 4; k += stride) {
+    if (is_int) {
+      const int4 v = reinterpret_cast<const int4 *>(g_static_batch)[k];
+      longlong2 *a = reinterpret_cast<longlong2 *>(acc) + 2 * k;
+      longlong2 a0 = a[0], a1 = a[1];
+      a0.x += v.x; a0.y += v.y; a1.x += v.z; a1.y += v.w;
+      a[0] = a0; a[1] = a1;
+    } else {
+      const float4 v = reinterpret_cast<const float4 *>(g_static_batch)[k];
+      double2 *a = reinterpret_cast<double2 *>(acc) + 2 * k;
+      double2 a0 = a[0], a1 = a[1];
+      a0.x += v.x; a0.y += v.y; a1.x += v.z; a1.y += v.w;
+      a[0] = a0; a[1] = a1;
+    }
+  }
+}
 
 namespace {
 
@@ -732,6 +759,55 @@ int corr_accumulate_wide(corr_handle *h, const void *d_in, void *d_acc, void *st
   if (fp.n % 4) return fail(CORR_EUNSUPPORTED, "corr_accumulate_wide: odd number of visibilities");
   const int blocks = static_cast<int>(std::min<long long>((fp.n / 4 + 255) / 256, static_cast<long long>(h->n_sms) * 8));
   corr::fold_wide_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(fp);
+  CUDA_TRY(cudaGetLastError());
+  return CORR_OK;
+}
+
+// Device address of g_static_batch on the CURRENT device, looked up once per device (each device that loads the
+// module has its own copy of the array at its own address).  Host-only bookkeeping; no device memory is allocated.
+static int static_batch_ptr(void **out) {
+  enum { kMaxDevices = 64 };
+  static void *ptr[kMaxDevices] = {};
+  static std::mutex mu;
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(CORR_EUNSUPPORTED, "corr_accumulate_wide_static: device ordinal %d not supported", dev);
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr[dev]) {
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_static_batch);
+    if (e != cudaSuccess || !p)
+      return fail(CORR_ECUDA, "corr_accumulate_wide_static: address of the static batch buffer on device %d: %s", dev,
+                  cudaGetErrorString(e));
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return CORR_OK;
+}
+
+// corr_accumulate_wide with the batch staged in g_static_batch instead of a handle-owned cudaMalloc'ed buffer: for
+// callers that cannot allocate (see include/corr.h for who they are, the size limit and the sharing rules).
+int corr_accumulate_wide_static(corr_handle *h, const void *d_in, void *d_acc, void *stream) {
+  if (!h || !d_in || !d_acc) return fail(CORR_EINVAL, "corr_accumulate_wide_static: NULL argument");
+  if (reinterpret_cast<uintptr_t>(d_acc) & 15) return fail(CORR_EINVAL, "corr_accumulate_wide_static: d_acc must be 16-byte aligned");
+  if (h->vis_bytes > static_cast<size_t>(CORR_STATIC_BATCH_BYTES))
+    return fail(CORR_EUNSUPPORTED,
+                "corr_accumulate_wide_static: one batch of visibilities is %zu bytes, the static buffer holds %u "
+                "(CORR_STATIC_BATCH_BYTES); use corr_accumulate_wide, which allocates its buffer",
+                h->vis_bytes, static_cast<unsigned>(CORR_STATIC_BATCH_BYTES));
+  if ((h->vis_bytes / 4) % 4) return fail(CORR_EUNSUPPORTED, "corr_accumulate_wide_static: odd number of visibilities");
+  void *d_batch = nullptr;
+  if (int rc = static_batch_ptr(&d_batch)) return rc;
+  // the batch is an ordinary overwriting integration: every element of the region used is written (sliced plans
+  // memset theirs on `stream` first), so the previous call's contents never reach the fold
+  const int acc_mode = h->accumulate;
+  h->accumulate = 0;
+  const int rc = corr_xengine(h, d_in, d_batch, stream);
+  h->accumulate = acc_mode;
+  if (rc != CORR_OK) return rc;
+  const long long n = static_cast<long long>(h->vis_bytes / 4);
+  const int blocks = static_cast<int>(std::min<long long>((n / 4 + 255) / 256, static_cast<long long>(h->n_sms) * 8));
+  fold_wide_static_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(d_acc, n, h->dtype != CORR_CF32);
   CUDA_TRY(cudaGetLastError());
   return CORR_OK;
 }
