@@ -782,10 +782,9 @@ def main():
         roof["fp32_probe_tflops"] = peaks["fp32_probe"]
     if roof["bound"] == "tensor":
         roof.update(tensor_fracs(w, kern, peaks))
-    if w.dtype != "ci8":
-        roof["kernel"] = "xengine_f32_n64_kernel" if w.n_inputs == 64 else "xengine_f32_kernel"
-    else:
-        roof["kernel"] = "xengine_i8_pair_kernel" if (w.n_inputs >= 512 or (w.n_inputs >= 256 and (w.n_time >= 2048 or w.n_time <= 1024))) else "xengine_i8_kernel"
+    plan = h.plan_info()      # the kernel and schedule the library planned (corr_plan_info), not a re-derivation
+    roof["kernel"] = plan["kernel"]
+    roof["plan"] = {k: plan[k] for k in ("gsize", "slices", "grid", "mixed", "stages", "wide", "resident")}
     roof["kernel_ms"] = kern * 1e3
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     traffic = json.load(open(tpath)).get(args.config) if os.path.exists(tpath) else None

@@ -117,7 +117,9 @@ long long corr_accumulate_count(const corr_handle *h);
  *   d_acc : device, [n_chan][N_I(N_I+1)/2] (int64 re, int64 im) for CORR_CI8 / CORR_CI4 -- exact for any
  *           number of batches -- or (double re, double im) for CORR_CF32; corr_acc_bytes(h) bytes,
  *           16-byte aligned, zeroed by the caller before the first batch.
- * Independent of corr_set_accumulate.  Asynchronous on `stream`.  Returns CORR_OK, CORR_EINVAL, CORR_EALLOC
+ * Independent of corr_set_accumulate.  Asynchronous on `stream`.  Every call on one handle stages its batch in the
+ * same handle-owned buffer: calls on ONE handle must be stream-ordered (one stream, or events between streams) --
+ * two accumulations double-buffered over two streams need two handles.  Returns CORR_OK, CORR_EINVAL, CORR_EALLOC
  * or CORR_ECUDA.  corr_normalize_wide is the read-out of d_acc (count = samples accumulated) into
  * (float re, float im), d_out of corr_vis_bytes(h) bytes.
  */
@@ -171,10 +173,12 @@ int corr_normalize(corr_handle *h, const void *d_vis, double count, void *d_out,
  * integration too small to fill the chip (config 1: 8 MB) costs a launch, a pipeline fill and one exposed
  * DRAM round trip per call; here the tile schedule spans all n inputs, so every SM streams for the whole call.
  *   d_in  : HOST array of n device pointers, each as corr_xengine's d_in
- *   d_vis : HOST array of n device pointers, each as corr_xengine's d_vis (distinct buffers)
+ *   d_vis : HOST array of n device pointers, each as corr_xengine's d_vis.  No d_vis[k] may overlap another entry's
+ *           d_vis or ANY entry's d_in (CORR_EINVAL, nothing enqueued): in the single launch all integrations run
+ *           at once.  Only in accumulate mode (call by call on `stream`) may several entries name one d_vis.
  *   n     : >= 1; more than 64 integrations are issued as several launches of <= 64
  * Same result as n corr_xengine calls (bit-exact for CI8).  The single-launch path covers CORR_CI8 shapes
- * that run on single CTAs (N_I <= 128, and 256 <= N_I < 512 with 1024 < T < 2048); every other
+ * that run on single CTAs (corr_plan_info: CORR_KERNEL_I8 -- N_I <= 192, and N_I < 512 with 1024 < T < 2048); every other
  * case (CTA-pair plans, CORR_CI4, CORR_CF32, the standalone corner turn, accumulate mode) falls back to n
  * ordinary calls on `stream`.  Returns as corr_xengine.
  */
@@ -197,7 +201,8 @@ int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
  */
 enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
                                    panels per work item and `slices` (1..64) time slices (slices = 0: only the
-                                   group width is forced); 0 = automatic                                     */
+                                   group width is forced, whatever the input size, corr_xengine_batch
+                                   included); 0 = automatic                                                 */
        CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned;
                                    2: CTA pairs from N_I = 128 up (experiments)                                 */
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
@@ -211,6 +216,25 @@ enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices force
        CORR_OPT_MIX = 9         /* 0: N_I <= 64 with more work groups than SMs: every group in the same number of time
                                    slices; 1 (default): whole groups plus sliced left-over groups                */ };
 int corr_set_option(corr_handle *h, int key, int value);
+
+/*
+ * corr_plan_info -- what the handle's current plan (corr_create, then every corr_set_option / corr_set_turn) will launch
+ * for corr_xengine; read-only, for benchmarks, profiles and tests that have to name the kernel and schedule they measured
+ * instead of re-deriving the planner's thresholds.  info: HOST array of CORR_PLAN_INFO_LEN ints indexed by CORR_PLAN_*;
+ * kernel: optional HOST buffer that receives the kernel's function name (NULL or kernel_len = 0 to skip).
+ */
+enum { CORR_PLAN_KERNEL = 0,  /* CORR_KERNEL_* below                                                          */
+       CORR_PLAN_GSIZE = 1,   /* N_I <= 64: adjacent panels (CI8 / CI4) or channels (CF32, N_I = 64) per work item; else 0 / 1 */
+       CORR_PLAN_SLICES = 2,  /* time slices per group (the sliced groups' count when CORR_PLAN_MIXED)        */
+       CORR_PLAN_GRID = 3,    /* CTAs per launch                                                             */
+       CORR_PLAN_MIXED = 4,   /* 1: whole groups plus sliced left-over groups                                */
+       CORR_PLAN_STAGES = 5,  /* depth of the TMA stage ring (int8 / 4-bit kernels)                          */
+       CORR_PLAN_WIDE = 6,    /* 1: the pair plan contains 512-wide tiles                                    */
+       CORR_PLAN_SMEM = 7,    /* dynamic shared memory per CTA, bytes (int8 / 4-bit kernels)                 */
+       CORR_PLAN_INFO_LEN = 8 };
+enum { CORR_KERNEL_I8 = 0, CORR_KERNEL_I8_PAIR = 1, CORR_KERNEL_I8_PAIR_RESIDENT = 2, CORR_KERNEL_I4 = 3,
+       CORR_KERNEL_F32 = 4, CORR_KERNEL_F32_N64 = 5 };
+int corr_plan_info(const corr_handle *h, int *info, char *kernel, size_t kernel_len);
 
 /*
  * corr_corner_turn -- the standalone corner-turn kernel, CI8 or CF32:

@@ -23,7 +23,7 @@ EXPORTS = ("corr_create", "corr_xengine", "corr_destroy", "corr_last_error", "co
            "corr_in_bytes", "corr_vis_bytes", "corr_launches_per_call", "corr_set_turn",
            "corr_corner_turn", "corr_stream_run", "corr_set_accumulate", "corr_accumulate_count", "corr_normalize",
            "corr_accumulate_wide", "corr_accumulate_wide_static", "corr_normalize_wide", "corr_acc_bytes", "corr_xengine_batch", "corr_set_chan_window",
-           "corr_set_option",
+           "corr_set_option", "corr_plan_info",
            "corr_fstage_create", "corr_fstage_run", "corr_fstage_destroy", "corr_fstage_in_bytes", "corr_fstage_out_bytes", "corr_stream_run_fx", "corr_fstage_set_input")
 # include/corr_diag.h (diagnostics, libcorr_diag.so only)
 DIAG_EXPORTS = ("corr_set_probe", "corr_probe_stats", "corr_probe_mma", "corr_probe_ffma")
@@ -72,6 +72,8 @@ def _bind(path, diag):
     L.corr_xengine_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ci, vp]
     L.corr_set_chan_window.restype, L.corr_set_chan_window.argtypes = ci, [vp, ci, ci]
     L.corr_set_option.restype, L.corr_set_option.argtypes = ci, [vp, ci, ci]
+    L.corr_plan_info.restype = ci
+    L.corr_plan_info.argtypes = [vp, ctypes.POINTER(ci), ctypes.c_char_p, ctypes.c_size_t]
     if diag:
         L.corr_set_probe.restype, L.corr_set_probe.argtypes = ci, [vp, ci]
         L.corr_probe_stats.restype, L.corr_probe_stats.argtypes = ci, [vp, ctypes.POINTER(ctypes.c_double)]
@@ -165,6 +167,18 @@ class Correlator:
     def set_option(self, key, value):
         if lib().corr_set_option(self._h, key, value) != CORR_OK:
             _raise()
+
+    def plan_info(self):
+        """corr_plan_info: {"kernel": name, "kernel_id", "gsize", "slices", "grid", "mixed", "stages", "wide", "smem"}."""
+        info = (ctypes.c_int * 8)()
+        name = ctypes.create_string_buffer(64)
+        if lib().corr_plan_info(self._h, info, name, 64) != CORR_OK:
+            _raise()
+        keys = ("kernel_id", "gsize", "slices", "grid", "mixed", "stages", "wide", "smem")
+        out = {k: int(info[i]) for i, k in enumerate(keys)}
+        out["kernel"] = name.value.decode()
+        out["resident"] = out["kernel_id"] == 2
+        return out
 
     def set_chan_window(self, n_chan_total, chan0):
         """Read channels chan0 .. chan0 + n_chan - 1 of a [T][n_chan_total][N] buffer in place."""

@@ -114,7 +114,8 @@ struct corr_handle {
   int n_inputs, n_chan, n_time, dtype;
   int n_chan_total, chan0;  // channel window (corr_set_chan_window): d_in is [T][n_chan_total][N], this handle owns chan0 .. chan0 + n_chan - 1
   long long n_baselines;
-  size_t in_bytes, vis_bytes;
+  size_t in_bytes, vis_bytes;  // buffer sizes (in_bytes: of the FULL cube when the handle owns a channel window)
+  size_t work_bytes;           // input bytes this handle actually reads per call: what the planner and the launch mode go by
   int n_sms;
   int turn_mode;
   int probe;
@@ -175,7 +176,8 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     const int G = h->n_sms;
     int best_g = 4, best_s = 1;
     double best_t = 1e30;
-    const bool small = h->in_bytes <= (64u << 20);
+    const bool small = h->work_bytes <= (64u << 20);
+    const int forced_g = h->opt_diag_plan >> 8;  // CORR_OPT_DIAG_PLAN: the group width is forced in every branch below
     if (n_batch > 1) {
       // batched launch: whole integrations (no zeroing nodes), the panel-group width that keeps the SMs evenly
       // loaded.  When one time row has no more panels than there are SMs, the CTAs working side by side consume
@@ -185,6 +187,7 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
       const bool rows_shared = ip.n_panels <= G;
       const double rate[5] = {0.0, rows_shared ? 1.0 : 0.70, rows_shared ? 1.0 : 0.92, 0.0, 1.0};
       for (int g = 1; g <= 4; g <<= 1) {
+        if (forced_g && g != forced_g) continue;
         const long long n = 1LL * ((ip.n_panels + g - 1) / g) * n_batch;
         const long long rounds = (n + G - 1) / G;
         const double t = rounds * g / rate[g];
@@ -192,6 +195,7 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
       }
     } else if (small) {
       for (int g = 4; g >= 1; g >>= 1) {
+        if (forced_g && g != forced_g) continue;
         const int base = (ip.n_panels + g - 1) / g;
         for (int s = 1; s <= 64; ++s) {
           int len = ((T + s - 1) / s + 63) / 64 * 64;
@@ -215,9 +219,8 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
       //   uniform plan: every group in s slices; mixed plan: a x G whole groups (plain stores, no zeroing) + the b
       //   left-over groups in s slices (c2: 148 whole + 44 groups in thirds).
       const double bw = 6.5e12 / G;
-      const int g_lo = (h->opt_diag_plan >> 8) ? (h->opt_diag_plan >> 8) : 2, g_hi = (h->opt_diag_plan >> 8) ? (h->opt_diag_plan >> 8) : 4;
+      const int g_lo = forced_g ? forced_g : 2, g_hi = forced_g ? forced_g : 4;
       for (int g = g_hi; g >= g_lo; g >>= 1) {
-        if (g == 1 && !(h->opt_diag_plan >> 8)) continue;
         const double ts = g * 128.0 / (bw * (g == 4 ? 1.0 : g == 2 ? 0.92 : 0.70));
         const double epi = g == 4 ? 4.0e-6 : 0.5e-6, epi_add = g == 4 ? 5.0e-6 : 1.0e-6;
         const int groups = (ip.n_panels + g - 1) / g;
@@ -330,7 +333,7 @@ void plan_f32(corr_handle *h, std::vector<int2> &items) {
     for (int I = 0; I < blocks; ++I)
       for (int J = 0; J <= I; ++J) items.push_back(make_int2(c, I | (J << 16)));
   h->n_items_f32 = static_cast<int>(items.size());
-  // N_I = 64: (8-channel group, time slice) units; as many slices as fill the SMs evenly (cost = rounds x rows per
+  // N_I = 64: (kN64Chan-channel group, time slice) units; as many slices as fill the SMs evenly (cost = rounds x rows per
   // slice, plus 32 rows for the zeroing node and the reduce-adds of a sliced plan)
   h->n64_groups = h->n64_slices = h->n64_slice_len = h->n64_full = 0;
   if (h->n_inputs == 64 && !h->opt_f32_generic) {
@@ -486,6 +489,7 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype) {
   h->chan0 = 0;
   h->n_baselines = static_cast<long long>(n_inputs) * (n_inputs + 1) / 2;
   h->in_bytes = static_cast<size_t>(n_time) * n_chan * n_inputs * sample_bytes(dtype);
+  h->work_bytes = h->in_bytes;
   h->vis_bytes = static_cast<size_t>(n_chan) * h->n_baselines * 8;
   h->n_sms = prop.multiProcessorCount;
   h->turn_mode = CORR_TURN_FUSED;
@@ -543,6 +547,38 @@ size_t corr_acc_bytes(const corr_handle *h) { return h ? 2 * h->vis_bytes : 0; }
 int corr_launches_per_call(const corr_handle *h) {
   if (!h) return 0;
   return (h->dtype == CORR_CI8 && h->turn_mode == CORR_TURN_STANDALONE) ? 2 : 1;  // kernels; a memset node precedes them when the integration is time-sliced
+}
+
+int corr_plan_info(const corr_handle *h, int *info, char *kernel, size_t kernel_len) {
+  if (!h || !info) return fail(CORR_EINVAL, "corr_plan_info: NULL argument");
+  for (int k = 0; k < CORR_PLAN_INFO_LEN; ++k) info[k] = 0;
+  const char *name;
+  if (h->dtype == CORR_CF32) {
+    const bool n64 = h->n64_groups > 0;
+    name = n64 ? "xengine_f32_n64_kernel" : "xengine_f32_kernel";
+    info[CORR_PLAN_KERNEL] = n64 ? CORR_KERNEL_F32_N64 : CORR_KERNEL_F32;
+    info[CORR_PLAN_GSIZE] = n64 ? corr::kN64Chan : 1;
+    info[CORR_PLAN_SLICES] = n64 ? h->n64_slices : 1;
+    info[CORR_PLAN_GRID] = n64 ? h->n64_full + (h->n64_groups - h->n64_full) * h->n64_slices : h->n_items_f32;
+    info[CORR_PLAN_MIXED] = n64 && h->n64_full > 0 && h->n64_full < h->n64_groups;
+  } else {
+    const corr::I8Params &ip = h->plan.ip;
+    const bool i4 = h->dtype == CORR_CI4;
+    name = i4 ? "xengine_i4_kernel" : ip.pair2 ? "xengine_i8_pair_kernel" : "xengine_i8_kernel";
+    info[CORR_PLAN_KERNEL] = i4 ? CORR_KERNEL_I4 : ip.pair2 ? (ip.resident ? CORR_KERNEL_I8_PAIR_RESIDENT : CORR_KERNEL_I8_PAIR) : CORR_KERNEL_I8;
+    info[CORR_PLAN_GSIZE] = ip.diag ? ip.gsize : 0;
+    info[CORR_PLAN_SLICES] = ip.mix_cut > 0 ? ip.mix_len ? (h->n_time + ip.mix_len - 1) / ip.mix_len : 1 : ip.n_slices;
+    info[CORR_PLAN_GRID] = h->plan.grid;
+    info[CORR_PLAN_MIXED] = ip.mix_cut > 0;
+    info[CORR_PLAN_STAGES] = ip.stages;
+    bool wide = false;
+    if (ip.pair2 && !ip.resident)
+      for (int k = 0; k < ip.n_kinds; ++k) wide = wide || ((ip.kinds[k] >> 11) & 1);
+    info[CORR_PLAN_WIDE] = wide;
+    info[CORR_PLAN_SMEM] = static_cast<int>(h->plan.smem);
+  }
+  if (kernel && kernel_len) snprintf(kernel, kernel_len, "%s", name);
+  return CORR_OK;
 }
 
 int corr_set_option(corr_handle *h, int key, int value) {
@@ -738,6 +774,8 @@ int corr_normalize_wide(corr_handle *h, const void *d_acc, double count, void *d
   return launch_normalize(h, d_acc, count, d_out, stream, (h && h->dtype == CORR_CF32) ? corr::kSumF64 : corr::kSumI64, "corr_normalize_wide");
 }
 
+static int xengine_impl(corr_handle *h, const void *d_in, void *d_vis, void *stream, const int accumulate);
+
 int corr_accumulate_wide(corr_handle *h, const void *d_in, void *d_acc, void *stream) {
   if (!h || !d_in || !d_acc) return fail(CORR_EINVAL, "corr_accumulate_wide: NULL argument");
   if (reinterpret_cast<uintptr_t>(d_acc) & 15) return fail(CORR_EINVAL, "corr_accumulate_wide: d_acc must be 16-byte aligned");
@@ -746,10 +784,7 @@ int corr_accumulate_wide(corr_handle *h, const void *d_in, void *d_acc, void *st
     if (e != cudaSuccess) return fail(CORR_EALLOC, "corr_accumulate_wide: batch buffer of %zu bytes: %s", h->vis_bytes, cudaGetErrorString(e));
   }
   // the batch itself is an ordinary overwriting integration (int32 / float sums of T samples cannot overflow)
-  const int acc_mode = h->accumulate;
-  h->accumulate = 0;
-  const int rc = corr_xengine(h, d_in, h->d_wide_vis, stream);
-  h->accumulate = acc_mode;
+  const int rc = xengine_impl(h, d_in, h->d_wide_vis, stream, 0);
   if (rc != CORR_OK) return rc;
   corr::FoldParams fp;
   fp.vis = h->d_wide_vis;
@@ -800,10 +835,7 @@ int corr_accumulate_wide_static(corr_handle *h, const void *d_in, void *d_acc, v
   if (int rc = static_batch_ptr(&d_batch)) return rc;
   // the batch is an ordinary overwriting integration: every element of the region used is written (sliced plans
   // memset theirs on `stream` first), so the previous call's contents never reach the fold
-  const int acc_mode = h->accumulate;
-  h->accumulate = 0;
-  const int rc = corr_xengine(h, d_in, d_batch, stream);
-  h->accumulate = acc_mode;
+  const int rc = xengine_impl(h, d_in, d_batch, stream, 0);
   if (rc != CORR_OK) return rc;
   const long long n = static_cast<long long>(h->vis_bytes / 4);
   const int blocks = static_cast<int>(std::min<long long>((n / 4 + 255) / 256, static_cast<long long>(h->n_sms) * 8));
@@ -876,13 +908,16 @@ static int accumulate_guard(corr_handle *h, long long batches) {
   return CORR_OK;
 }
 
-int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
+// One integration; `accumulate` != 0 adds into d_vis (accumulate mode) instead of overwriting.  The flag is an argument so
+// that callers which need an overwriting integration (the wide accumulators' batch) do not have to flip the handle's state.
+static int xengine_impl(corr_handle *h, const void *d_in, void *d_vis, void *stream, const int accumulate) {
   if (!h) return fail(CORR_EINVAL, "corr_xengine: NULL handle");
   if (!d_in || !d_vis) return fail(CORR_EINVAL, "corr_xengine: NULL device pointer");
   if ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_vis)) & 15)
     return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis must be 16-byte aligned");
   if (d_in == d_vis) return fail(CORR_EINVAL, "corr_xengine: d_in and d_vis alias");
-  if (int rc = accumulate_guard(h, 1)) return rc;
+  if (accumulate)
+    if (int rc = accumulate_guard(h, 1)) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (h->dtype == CORR_CF32) {
     if (h->n64_groups > 0) {
@@ -893,8 +928,8 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
       np.n_chan_total = h->n_chan_total; np.chan0 = h->chan0;
       np.n_groups = h->n64_groups; np.n_slices = h->n64_slices; np.slice_len = h->n64_slice_len;
       np.n_full = h->n64_full;
-      np.add = h->accumulate ? 1 : 0;
-      if (h->n64_slices > 1 && !h->accumulate) {  // the sliced groups' channels are zeroed: their slices reduce-add
+      np.add = accumulate ? 1 : 0;
+      if (h->n64_slices > 1 && !accumulate) {  // the sliced groups' channels are zeroed: their slices reduce-add
         const size_t chan0 = static_cast<size_t>(h->n64_full) * corr::kN64Chan;
         const size_t off = chan0 * h->n_baselines * 8;
         CUDA_TRY(cudaMemsetAsync(static_cast<char *>(d_vis) + off, 0, h->vis_bytes - off, st));
@@ -902,7 +937,7 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
       const int units = h->n64_full + (h->n64_groups - h->n64_full) * h->n64_slices;
       corr::xengine_f32_n64_kernel<<<units, corr::kN64Threads, corr::kN64Smem, st>>>(np);
       CUDA_TRY(cudaGetLastError());
-      if (h->accumulate) ++h->acc_count;
+      if (accumulate) ++h->acc_count;
       return CORR_OK;
     }
     corr::F32Params fp;
@@ -916,10 +951,10 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     fp.n_chan_total = h->n_chan_total;
     fp.chan0 = h->chan0;
     fp.n_baselines = h->n_baselines;
-    fp.accumulate = h->accumulate;
+    fp.accumulate = accumulate;
     corr::xengine_f32_kernel<<<h->n_items_f32, h->f32_threads, 0, st>>>(fp);
     CUDA_TRY(cudaGetLastError());
-    if (h->accumulate) ++h->acc_count;
+    if (accumulate) ++h->acc_count;
     return CORR_OK;
   }
   const bool turned = h->turn_mode == CORR_TURN_STANDALONE;
@@ -940,9 +975,9 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
   ip.probe = h->probe;
   ip.diag_stats = h->d_diag_stats;
   ip.out_shift = h->dtype == CORR_CI4 ? 8 : 0;
-  ip.accumulate = h->accumulate;
+  ip.accumulate = accumulate;
   ip.collect = h->opt_collect;
-  if (h->plan.zero_vis && !h->accumulate) {  // slices accumulate with red.add
+  if (h->plan.zero_vis && !accumulate) {  // slices accumulate with red.add
     const size_t off = static_cast<size_t>(std::min(h->plan.zero_from_chan, h->n_chan)) * h->n_baselines * 8;
     CUDA_TRY(cudaMemsetAsync(static_cast<char *>(d_vis) + off, 0, h->vis_bytes - off, st));
   }
@@ -956,7 +991,7 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     // enough to hide that (c2: 160.7 -> 158.6 us call by call).
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (h->opt_pdl && cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cap = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
-    if (h->opt_pdl == 2 || (h->opt_pdl && (cap == cudaStreamCaptureStatusActive || h->in_bytes > (64u << 20)))) {
+    if (h->opt_pdl == 2 || (h->opt_pdl && (cap == cudaStreamCaptureStatusActive || h->work_bytes > (64u << 20)))) {
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3(grid); cfg.blockDim = dim3(corr::kI8Threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
       cudaLaunchAttribute attr[1];
@@ -969,8 +1004,13 @@ int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
     }
   }
   CUDA_TRY(cudaGetLastError());
-  if (h->accumulate) ++h->acc_count;
+  if (accumulate) ++h->acc_count;
   return CORR_OK;
+}
+
+int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream) {
+  if (!h) return fail(CORR_EINVAL, "corr_xengine: NULL handle");
+  return xengine_impl(h, d_in, d_vis, stream, h->accumulate);
 }
 
 int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_vis, int n, void *stream) {
@@ -981,6 +1021,31 @@ int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_v
     if ((reinterpret_cast<uintptr_t>(d_in[k]) | reinterpret_cast<uintptr_t>(d_vis[k])) & 15)
       return fail(CORR_EINVAL, "corr_xengine_batch: d_in[%d] and d_vis[%d] must be 16-byte aligned", k, k);
     if (d_in[k] == d_vis[k]) return fail(CORR_EINVAL, "corr_xengine_batch: d_in[%d] and d_vis[%d] alias", k, k);
+  }
+  // No output may overlap an input of the batch (any entry's), and outputs may not overlap one another: in the single
+  // launch all integrations run concurrently.  Sorted by start address, an interval overlaps an earlier one iff it starts
+  // before that one ends.  Accumulate mode runs call by call on `stream`, where several entries adding into one d_vis is
+  // well defined, so only there outputs may repeat.  Inputs may repeat freely (they are only read).
+  if (n > 1) {
+    struct Range { uintptr_t lo, hi; int is_vis, k; };
+    std::vector<Range> r;
+    r.reserve(2 * static_cast<size_t>(n));
+    for (int k = 0; k < n; ++k) {
+      const uintptr_t a = reinterpret_cast<uintptr_t>(d_in[k]), v = reinterpret_cast<uintptr_t>(d_vis[k]);
+      r.push_back({a, a + h->in_bytes, 0, k});
+      r.push_back({v, v + h->vis_bytes, 1, k});
+    }
+    std::sort(r.begin(), r.end(), [](const Range &x, const Range &y) { return x.lo < y.lo; });
+    uintptr_t end_vis = 0, end_in = 0;
+    int k_vis = -1, k_in = -1;
+    for (const Range &x : r) {
+      if (x.lo < end_vis && (!x.is_vis || !h->accumulate))
+        return fail(CORR_EINVAL, "corr_xengine_batch: %s[%d] overlaps d_vis[%d]", x.is_vis ? "d_vis" : "d_in", x.k, k_vis);
+      if (x.is_vis && x.lo < end_in)
+        return fail(CORR_EINVAL, "corr_xengine_batch: d_vis[%d] overlaps d_in[%d]", x.k, k_in);
+      if (x.is_vis) { if (x.hi > end_vis) { end_vis = x.hi; k_vis = x.k; } }
+      else if (x.hi > end_in) { end_in = x.hi; k_in = x.k; }
+    }
   }
   // single-launch path: CI8 on single CTAs, fused corner turn, overwrite semantics; everything else = n ordinary calls
   const bool one_launch = h->dtype == CORR_CI8 && !h->plan.ip.pair2 && h->turn_mode == CORR_TURN_FUSED && !h->accumulate && n > 1;
