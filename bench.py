@@ -81,6 +81,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index=0, period=0.01):
         super().__init__(daemon=True)
         self.period, self.samples, self.reasons, self.stop_flag = period, [], set(), False
+        self.power_w = []
         self.max_mhz = None
         try:
             import pynvml
@@ -101,6 +102,10 @@ class ClockSampler(threading.Thread):
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
                 try:
+                    self.power_w.append(nv.nvmlDeviceGetPowerUsage(self.dev) / 1000.0)
+                except Exception:
+                    pass
+                try:
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev)
                 except Exception:
                     r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
@@ -114,8 +119,11 @@ class ClockSampler(threading.Thread):
     def summary(self):
         s = sorted(self.samples)
         busy = [x for x in s if self.max_mhz is None or x > 0.3 * self.max_mhz] or s
-        return {"sm_mhz": busy[len(busy) // 2] if busy else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(r for r in self.reasons if r not in ("GpuIdle", "None", "All"))}
+        out = {"sm_mhz": busy[len(busy) // 2] if busy else None, "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(r for r in self.reasons if r not in ("GpuIdle", "None", "All"))}
+        if self.power_w:
+            out["power_w_max"] = round(max(self.power_w), 1)
+        return out
 
 
 def make_inputs(w, n_buffers, torch, rank=0):
@@ -392,10 +400,20 @@ def run_reference(args, w):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int64" if w.dtype == "ci8" else "f64", "data": "synthetic",
-            "config": {"workload": workload_name(w)},
+            "config": product_config(w, 1, "weak", 1),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def product_config(w, world, scaling, n_buffers):
+    """The `config` object of the JSON line; both arms (--impl b200 / reference) print the same one for the same command."""
+    return {"workload": workload_name(w), "n_inputs": w.n_inputs, "n_chan": w.n_chan, "n_time": w.n_time,
+            "parallelism": (f"channels sharded over {world} GPUs, each reading its window of the one cube in place (corr_set_chan_window)"
+                            if (world > 1 and scaling == "strong") else
+                            f"channel-independent replicas x{world}" if world > 1 else "single GPU"),
+            "l2": (f"input {w.in_bytes / 1e6:.0f} MB per step > 126 MB L2, no flush needed" if n_buffers == 1
+                   else f"rotating {n_buffers} distinct input buffers ({n_buffers * w.in_bytes / 1e6:.0f} MB > L2)")}
 
 
 def workload_name(w):
@@ -494,7 +512,7 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     if w.dtype == "cf32":
         out["fp32_peak_tflops"] = fp32_peak_flops(peaks) / 1e12
         out["fp32_peak_source"] = peaks["fp32_source"]
-        out["kernel"] = "xengine_f32_n64_kernel" if w.n_inputs == 64 else "xengine_f32_kernel"
+    out["kernel"] = r["handle"].plan_info()["kernel"]
     if key in ("c2", "c4"):
         out["corner_turn"] = corner_turn_entry(pkg, torch, w, r["handle"], r["bufs"][0])
     if "isolated_s" in r and "graph_s" not in r:
@@ -548,6 +566,105 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     del r
     torch.cuda.empty_cache()
     return out
+
+
+def sustained_entry(pkg, torch, key, peaks, seconds=2.0, block=25):
+    """The SUSTAINED regime of a tensor-bound config: >= `seconds` of back-to-back corr_xengine calls, CUDA events every
+    `block` calls, SM clock / power / throttle reasons sampled through NVML meanwhile.  Under the power cap the SM clock
+    falls well below its maximum; this is the regime MEASURED_PEAKS.json's bf16_tflops_sustained was measured in, so
+    frac_sustained divides by 2 x that figure and is only ever quoted with the clock record beside it.  The first
+    quarter of the loop (clock still settling) is left out of ms."""
+    import corrgen
+    w = corrgen.CONFIGS[key]
+    h = pkg.corr_create(w.n_inputs, w.n_chan, w.n_time, w.dtype)
+    n_buf = 1 if w.in_bytes > 2 * L2_BYTES else min(8, -(-3 * L2_BYTES // w.in_bytes))
+    bufs = make_inputs(w, n_buf, torch)
+    vis = h.empty_vis()
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for k in range(3):
+        h.xengine(bufs[k % n_buf], vis, stream)
+    e0.record(stream)
+    for k in range(10):
+        h.xengine(bufs[k % n_buf], vis, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    est = e0.elapsed_time(e1) * 1e-3 / 10
+    n_blocks = max(8, int(seconds / (est * block)) + 1)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(n_blocks + 1)]
+    sampler = ClockSampler(index=torch.cuda.current_device(), period=0.02)
+    time.sleep(0.2)
+    sampler.start()
+    ev[0].record(stream)
+    for b in range(n_blocks):
+        for k in range(block):
+            h.xengine(bufs[k % n_buf], vis, stream)
+        ev[b + 1].record(stream)
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join(timeout=1.0)
+    total = ev[0].elapsed_time(ev[n_blocks]) * 1e-3
+    q = n_blocks // 4
+    settled = ev[q].elapsed_time(ev[n_blocks]) * 1e-3 / ((n_blocks - q) * block)
+    first = ev[0].elapsed_time(ev[1]) * 1e-3 / block
+    t_a, t_b = roofline_times(w, peaks)
+    ops = 8.0 * w.cmacs
+    burst, sus = 2.0 * peaks["bf16_tflops"] * 1e12, 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * 1e12
+    out = {"loop_s": total, "calls": n_blocks * block, "ms": settled * 1e3, "ms_first_block": first * 1e3,
+           "frac_sustained": max(w.in_bytes / (peaks["hbm_gbs"] * 1e9), ops / sus) / settled,
+           "frac_burst": max(w.in_bytes / (peaks["hbm_gbs"] * 1e9), ops / burst) / settled,
+           "denominators": "2 x bf16_tflops_sustained / 2 x bf16_tflops (burst) of MEASURED_PEAKS.json, or input bytes / hbm_gbs if larger",
+           "clocks": sampler.summary()}
+    h.destroy()
+    del bufs, vis
+    torch.cuda.empty_cache()
+    return out
+
+
+def _r(x, n=4):
+    return None if x is None else float(f"{x:.{n}g}")
+
+
+def summary_of(line):
+    """Every config's headline figures in < 1.5 KB, written LAST in the JSON line so that a record which keeps only the tail
+    of stdout still holds them.  frac_* are fractions of the relevant roofline = max(input bytes / measured HBM bandwidth,
+    8 ops x CMACs / peak): burst = loop of ms-scale calls against 2 x bf16 burst, iso = one call on an idle device against
+    the same, sus = the >= 2 s loop against 2 x bf16 sustained (its SM clock and power are in by_config.*.sustained)."""
+    by = line.get("by_config", {})
+    roof = line["roofline"]
+    cpu = line.get("cpu_baseline", {})
+    s = {"c2": {"ms": _r(line["ms_per_step"]), "frac_burst": _r(roof["frac"]), "parity": cpu.get("parity")}}
+    c1 = by.get("c1", {})
+    if "ms" in c1:
+        s["c1"] = {"ms_graph": _r(c1["ms"]), "frac_graph": _r(c1["frac"]), "ms_b32": _r(c1.get("ms_batched")),
+                   "frac_b32": _r(c1.get("frac_batched")), "ms_b64": _r(c1.get("ms_batched64")), "frac_b64": _r(c1.get("frac_batched64")),
+                   "b_eq_single": c1.get("batched_equals_single_calls")}
+    for key in ("c3", "c4"):
+        e = by.get(key, {})
+        if "ms" not in e:
+            continue
+        s[key] = {"ms": _r(e["ms"]), "frac_burst": _r(e.get("frac_2xbf16_roofline")), "ms_iso": _r(e.get("ms_isolated")),
+                  "frac_iso": _r(e.get("frac_2xbf16_roofline_isolated")), "kernel": e.get("kernel")}
+        su = e.get("sustained", {})
+        if "ms" in su:
+            s[key].update({"ms_sus": _r(su["ms"]), "frac_sus": _r(su["frac_sustained"]), "sus_mhz": su["clocks"].get("sm_mhz"),
+                           "sus_w": su["clocks"].get("power_w_max"), "sus_reasons": su["clocks"].get("reasons")})
+    c5 = by.get("c5", {})
+    if "ms" in c5:
+        st = c5.get("stream", {})
+        par = st.get("parity", {})
+        s["c5"] = {"ms": _r(c5["ms"]), "frac_fp32": _r(c5["frac"]), "rtf": _r(st.get("rtf_vs_15.36MSps")),
+                   "h2d_gbs": _r(st.get("h2d_gbs")), "stream_parity": par.get("result") if isinstance(par, dict) else par}
+    for key in ("c2_4bit", "c3_shape_4bit", "c5_fstage"):
+        e = by.get(key, {})
+        if "ms" in e:
+            s[key] = {"ms": _r(e["ms"]), "frac": _r(e["frac"])}
+    curve = by.get("vs_n_inputs")
+    if isinstance(curve, dict):
+        curve = curve.get("points")
+    if isinstance(curve, list):
+        s["vs_n_inputs_frac_burst"] = {str(p["n_inputs"]): _r(p["frac_burst"], 3) for p in curve if "frac_burst" in p}
+    return s
 
 
 def curve_entry(pkg, torch, peaks, steps=10, warmup=3):
@@ -789,17 +906,14 @@ def main():
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     traffic = json.load(open(tpath)).get(args.config) if os.path.exists(tpath) else None
     roof["traffic"] = traffic
+    roof["traffic_source"] = ("profiles/traffic.json: dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
+                              "capture of this kernel (not measured in this run)") if traffic is not None else None
 
     total_cmacs = w_full.cmacs if (args.scaling == "strong" and world > 1) else world * w.cmacs
     line = {"metric": METRIC, "value": total_cmacs / sec, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak",
             "vs_baseline": None, "dtype": "s8 x s8 -> s32" if w.dtype == "ci8" else "f32", "data": "synthetic",
-            "config": {"workload": workload_name(w), "n_inputs": w.n_inputs, "n_chan": w.n_chan, "n_time": w.n_time,
-                       "parallelism": (f"channels sharded over {world} GPUs, each reading its window of the one cube in place (corr_set_chan_window)"
-                                       if (world > 1 and args.scaling == "strong") else
-                                       f"channel-independent replicas x{world}" if world > 1 else "single GPU"),
-                       "l2": (f"input {w.in_bytes / 1e6:.0f} MB per step > 126 MB L2, no flush needed" if r["n_buffers"] == 1
-                              else f"rotating {r['n_buffers']} distinct input buffers ({r['n_buffers'] * w.in_bytes / 1e6:.0f} MB > L2)")},
+            "config": product_config(w, world, args.scaling, r["n_buffers"]),
             "clocks": sampler.summary() if sampler else None,
             "e2e": e2e, "gpu_launches": r["launches"], "roofline": roof,
             "graph_ms_per_step": graph_ms}
@@ -838,7 +952,14 @@ def main():
             sweep["vs_n_inputs"] = curve_entry(pkg, torch, peaks)
         except Exception as e:
             sweep["vs_n_inputs"] = {"error": str(e)[:200]}
+        for key in ("c3", "c4"):   # the seconds-long regime, with its clock record (runs last: it heats the chip)
+            if isinstance(sweep.get(key), dict) and "ms" in sweep[key]:
+                try:
+                    sweep[key]["sustained"] = sustained_entry(pkg, torch, key, peaks)
+                except Exception as e:
+                    sweep[key]["sustained"] = {"error": str(e)[:200]}
         line["by_config"] = sweep
+        line["summary"] = summary_of(line)
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
