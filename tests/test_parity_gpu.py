@@ -170,7 +170,9 @@ def test_corner_turn_is_the_permutation(pkg, dtype, N, C, T):
     assert np.array_equal(out.reshape(want.shape), want)
 
 
-CF32_SHAPES = [(64, 3, 50), (64, 2, 500), (64, 40, 17), (32, 3, 33), (96, 2, 20), (128, 2, 40), (192, 1, 30)]
+CF32_SHAPES = [(64, 3, 50), (64, 2, 500), (64, 40, 17), (32, 3, 33), (96, 2, 20), (128, 2, 40), (192, 1, 30),
+               # the generic kernel's many-block rows and diagonals: corr_create admits CF32 up to N_I = 4096
+               (256, 2, 40), (512, 1, 30), (1024, 1, 20), (2048, 1, 4)]
 
 
 @pytest.mark.parametrize("N,C,T", CF32_SHAPES)
