@@ -73,6 +73,9 @@ corr_handle *corr_create(int n_inputs, int n_chan, int n_time, int dtype);
  *   d_vis : device, [n_chan][N_I(N_I+1)/2] interleaved complex (int32 or float pairs),
  *           OVERWRITTEN with the raw sums of this call (reading R4); 16-byte aligned;
  *           must not alias d_in.  Im of every autocorrelation is exactly 0.
+ * An integration that does not fill the chip (config 1: 8 MB) is LATENCY-bound through this call -- a launch, a
+ * pipeline fill and one exposed DRAM round trip per call, 0.2 of the HBM roofline however it is enqueued; the
+ * throughput path for such inputs is corr_xengine_batch below (0.8 of the roofline at 32 integrations per launch).
  * Returns CORR_OK, CORR_EINVAL (NULL / misaligned pointers, NULL handle) or CORR_ECUDA.
  */
 int corr_xengine(corr_handle *h, const void *d_in, void *d_vis, void *stream);
