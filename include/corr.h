@@ -199,21 +199,19 @@ int corr_xengine_batch(corr_handle *h, const void *const *d_in, void *const *d_v
 int corr_set_chan_window(corr_handle *h, int n_chan_total, int chan0);
 
 /*
- * corr_set_option -- plan knobs for A/B measurements and tests.  Each call re-plans
- * the handle; the defaults are what corr_create chose.  CORR_EINVAL for an unknown key or a value out of range.
+ * corr_set_option -- forces a plan family, for the tests that must reach every schedule and for measurements
+ * (DESIGN.md section 7).  Each call re-plans the handle; the defaults are what corr_create chose.  CORR_EINVAL for an
+ * unknown key or a value out of range.  The keys below are the supported ones; the experiment switches of the
+ * where-the-time-goes study (CTA count, dependent launches, collector reuse, CTA pairs below N_I = 256) are declared in
+ * corr_diag.h and are no part of this ABI.
  */
 enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices forces `gsize` (1, 2, 4) adjacent
                                    panels per work item and `slices` (1..64) time slices (slices = 0: only the
                                    group width is forced, whatever the input size, corr_xengine_batch
                                    included); 0 = automatic                                                 */
-       CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned;
-                                   2: CTA pairs from N_I = 128 up (experiments)                                 */
+       CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
-       CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
-       CORR_OPT_PDL = 6,        /* programmatic dependent launch of the single-CTA int8 kernel: 0 never; 1 (default) inside a
-                                   stream capture and for inputs above 64 MB; 2 always                           */
-       CORR_OPT_COLLECT = 7,    /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */
        CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 256, T <= 1024: a CTA keeps its A panel of the whole
                                    integration in shared memory); 1 (default)                                 */
        CORR_OPT_MIX = 9         /* 0: N_I <= 64 with more work groups than SMs: every group in the same number of time

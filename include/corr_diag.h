@@ -18,6 +18,17 @@ extern "C" {
 #endif
 
 /*
+ * Experiment keys of corr_set_option (corr.h): A/B switches of the where-the-time-goes study, kept out of the product
+ * header because no user of the library needs them.  Both builds accept them -- the parity tests force these paths in
+ * the product kernels (tests/test_parity_gpu.py, tests/test_fuzz_gpu.py) -- but they may change or go without notice.
+ */
+enum { CORR_OPT_UNITS = 4,      /* > 0: at most that many CTAs walk the schedule (single-CTA plans); 0 = all SMs */
+       CORR_OPT_PDL = 6,        /* programmatic dependent launch of the single-CTA int8 kernel: 0 never; 1 (default) inside a
+                                   stream capture and for inputs above 64 MB; 2 always                           */
+       CORR_OPT_COLLECT = 7     /* 0: 512-wide pair tiles read A twice per k-step; 1 (default): collector reuse */ };
+/* CORR_OPT_PAIRS = 2: CTA pairs from N_I = 128 up (the supported values 0 | 1 are in corr.h) */
+
+/*
  * corr_set_probe -- switches engines of the CI8 kernel off so that the others can be timed alone.  Bit
  * mask: 1 = skip the MMAs, 2 = skip the TMA loads (producer only hand-shakes), 4 = no epilogue, 8 = no
  * producer and no stage hand-shake at all, 16 = epilogue without its global stores, 128 = results stay correct, the

@@ -2,9 +2,7 @@
 // Plans the tile schedule (descendant of the paper's constant-memory pair lookup table,
 // PAPER.md:117), encodes TMA tensor maps, launches the sm_100a kernels.  No CPU compute path.
 #include "../../include/corr.h"
-#ifdef CORR_DIAG
-#include "../../include/corr_diag.h"
-#endif
+#include "../../include/corr_diag.h"  // the experiment keys of corr_set_option; its entry points are compiled under CORR_DIAG only
 
 #include <cuda.h>
 #include <cuda_runtime.h>
