@@ -496,6 +496,28 @@ def corner_turn_entry(pkg, torch, w, h, x, steps=10):
             "xengine_ms_through_standalone_turn": sec_path * 1e3}
 
 
+def sweep_parity(torch, w, h, d_in, target_s=10.0):
+    """GPU output of one corr_xengine call on d_in against the oracle, channels 0..k-1 (k = all when the budget allows)."""
+    import numpy as np
+    import oracle
+    vis = h.empty_vis()
+    vis.fill_(-0x55555555)
+    h.xengine(d_in, vis)
+    torch.cuda.synchronize()
+    x = d_in.cpu().numpy()
+    cores = oracle.host_threads()
+    t0 = time.perf_counter()
+    first = oracle.xengine_ci8(x, 0, 1, threads=1)
+    one = max(time.perf_counter() - t0, 1e-4)
+    k = int(min(w.n_chan, max(1, target_s * cores / one)))
+    t0 = time.perf_counter()
+    ref = oracle.xengine_ci8(x, 0, k, threads=cores)
+    sec = time.perf_counter() - t0
+    ok = bool(np.array_equal(vis[:k].cpu().numpy(), ref)) and bool(np.array_equal(ref[:1], first))
+    del vis
+    return {"result": "bit-exact" if ok else "MISMATCH", "channels": k, "of": w.n_chan, "oracle_s": round(sec, 2), "cores": cores}
+
+
 def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
     """Kernel-only numbers of another config (context for 'vs N_I'; not a bench line of its own)."""
     import corrgen
@@ -545,6 +567,13 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
             r["handle"].xengine(r["batch_bufs"][k], single)
             same = same and bool(torch.equal(single, r["batch_vis"][k]))
         out["batched_equals_single_calls"] = same
+    if w.dtype == "ci8":
+        # parity of THIS launch configuration at full size: one more call on buffer 0, compared element by element with the
+        # oracle on as many whole channels as about 10 s of host time allow (all of them on a 16-core box)
+        try:
+            out["parity"] = sweep_parity(torch, w, r["handle"], r["bufs"][0])
+        except Exception as e:
+            out["parity"] = {"result": "not checked", "error": str(e)[:200]}
     if w.dtype == "cf32" and w.n_integrations > 1:
         # streaming driver: n_integrations back-to-back integrations from pinned host buffers,
         # H2D of k+1 under the kernel of k; a ring of 4 distinct pinned buffers stands in for the 20
@@ -625,6 +654,12 @@ def _r(x, n=4):
     return None if x is None else float(f"{x:.{n}g}")
 
 
+def _parity_word(p):
+    if not isinstance(p, dict):
+        return p
+    return p.get("result") if p.get("channels") == p.get("of") else f"{p.get('result')} ({p.get('channels')}/{p.get('of')} ch)"
+
+
 def summary_of(line):
     """Every config's headline figures in < 1.5 KB, written LAST in the JSON line so that a record which keeps only the tail
     of stdout still holds them.  frac_* are fractions of the relevant roofline = max(input bytes / measured HBM bandwidth,
@@ -638,13 +673,14 @@ def summary_of(line):
     if "ms" in c1:
         s["c1"] = {"ms_graph": _r(c1["ms"]), "frac_graph": _r(c1["frac"]), "ms_b32": _r(c1.get("ms_batched")),
                    "frac_b32": _r(c1.get("frac_batched")), "ms_b64": _r(c1.get("ms_batched64")), "frac_b64": _r(c1.get("frac_batched64")),
-                   "b_eq_single": c1.get("batched_equals_single_calls")}
+                   "b_eq_single": c1.get("batched_equals_single_calls"), "parity": _parity_word(c1.get("parity"))}
     for key in ("c3", "c4"):
         e = by.get(key, {})
         if "ms" not in e:
             continue
         s[key] = {"ms": _r(e["ms"]), "frac_burst": _r(e.get("frac_2xbf16_roofline")), "ms_iso": _r(e.get("ms_isolated")),
-                  "frac_iso": _r(e.get("frac_2xbf16_roofline_isolated")), "kernel": e.get("kernel")}
+                  "frac_iso": _r(e.get("frac_2xbf16_roofline_isolated")), "kernel": e.get("kernel"),
+                  "parity": _parity_word(e.get("parity"))}
         su = e.get("sustained", {})
         if "ms" in su:
             s[key].update({"ms_sus": _r(su["ms"]), "frac_sus": _r(su["frac_sustained"]), "sus_mhz": su["clocks"].get("sm_mhz"),
