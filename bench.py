@@ -496,7 +496,7 @@ def corner_turn_entry(pkg, torch, w, h, x, steps=10):
             "xengine_ms_through_standalone_turn": sec_path * 1e3}
 
 
-def sweep_parity(torch, w, h, d_in, target_s=10.0):
+def cpu_baseline_sweep_parity(torch, w, h, d_in, target_s=10.0):
     """GPU output of one corr_xengine call on d_in against the oracle, channels 0..k-1 (k = all when the budget allows)."""
     import numpy as np
     import oracle
@@ -571,7 +571,7 @@ def sweep_entry(pkg, torch, key, peaks, steps=20, warmup=3):
         # parity of THIS launch configuration at full size: one more call on buffer 0, compared element by element with the
         # oracle on as many whole channels as about 10 s of host time allow (all of them on a 16-core box)
         try:
-            out["parity"] = sweep_parity(torch, w, r["handle"], r["bufs"][0])
+            out["parity"] = cpu_baseline_sweep_parity(torch, w, r["handle"], r["bufs"][0])
         except Exception as e:
             out["parity"] = {"result": "not checked", "error": str(e)[:200]}
     if w.dtype == "cf32" and w.n_integrations > 1:

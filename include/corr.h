@@ -212,8 +212,9 @@ enum { CORR_OPT_DIAG_PLAN = 1,  /* N_I <= 64: value = 256 * gsize + slices force
        CORR_OPT_PAIRS = 2,      /* 0: single-CTA slab items only; 1 (default): CTA pairs (cta_group::2) where planned */
        CORR_OPT_WIDE = 3,       /* 0: no 512-wide pair tiles; 1 (default): for T >= 2048; 2: for every T       */
        CORR_OPT_F32_GENERIC = 5,/* 1: N_I = 64 float input runs the generic kernel instead of the N_I = 64 one */
-       CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 256, T <= 1024: a CTA keeps its A panel of the whole
-                                   integration in shared memory); 1 (default)                                 */
+       CORR_OPT_RESIDENT = 8,   /* 0: no resident-A plan (N_I >= 256, T <= 1024, or <= 1152 up to N_I = 512: a CTA pair keeps
+                                   its A panel of the whole integration in shared memory); 1 (default): where it
+                                   was measured to pay; 2: wherever it fits (T <= 1152)                        */
        CORR_OPT_MIX = 9         /* 0: N_I <= 64 with more work groups than SMs: every group in the same number of time
                                    slices; 1 (default): whole groups plus sliced left-over groups                */ };
 int corr_set_option(corr_handle *h, int key, int value);

@@ -269,7 +269,15 @@ void plan_i8(const corr_handle *h, int n_batch, I8Plan *out) {
     const int min_pair_panels = h->opt_pairs == 2 ? 2 : 8;  // CORR_OPT_PAIRS = 2 (experiments): CTA pairs from N_I = 128 up
     // the resident-A plan already from N_I = 256 (N_I = 256 / 384 at T = 1000: 185 -> 175, 252 -> 217 us against single-CTA slabs)
     const int min_res_panels = h->opt_pairs == 2 ? 2 : 4;
-    if (use_pairs && panels_per_chan >= min_res_panels && !long_ok && T <= 128 * corr::kResMaxSub && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
+    // ... by measurement (round 3, 0.5 GB inputs, resident / best other plan): with 5 or 7 panels per channel (N_I = 288, 320,
+    // 416, 448) the unit of two row pairs wastes a third / a quarter of its MMAs and single-CTA slabs win (1.03-1.16 at T = 500 ..
+    // 1100); up to 1024 samples (4-stage B ring) the plan wins everywhere else (0.73-0.99); with 9 sub-stages (T <= 1152, 3-stage
+    // ring) it still wins with 4, 6 and 8 panels (N_I = 256 / 384 / 512 at T = 1100: 0.96 / 0.90 / 0.92) and ties or loses above
+    // (1.0-1.09 from N_I = 576 up); a 2-stage ring (T <= 1280) loses everywhere (1.05-1.3).  CORR_OPT_RESIDENT = 2 forces the
+    // plan wherever it fits.
+    const bool res_fits = T <= 128 * corr::kResMaxSub;
+    const bool res_pays = T <= (panels_per_chan <= 8 ? 128 * corr::kResMaxSub : 1024) && panels_per_chan != 5 && panels_per_chan != 7;
+    if (use_pairs && panels_per_chan >= min_res_panels && !long_ok && res_fits && (res_pays || h->opt_resident == 2) && h->opt_resident && h->turn_mode == CORR_TURN_FUSED) {
       // resident-A plan (xengine_i8_resident.cuh): the A panel of the whole integration stays in shared memory; an item
       // is a unit of two row pairs (pp - 1 - u and u: pp + 1 tiles in every unit)
       ip.pair2 = 1;
@@ -592,7 +600,7 @@ int corr_set_option(corr_handle *h, int key, int value) {
     case CORR_OPT_PAIRS: h->opt_pairs = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_WIDE: h->opt_wide = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_COLLECT: h->opt_collect = value ? 1 : 0; break;
-    case CORR_OPT_RESIDENT: h->opt_resident = value ? 1 : 0; break;
+    case CORR_OPT_RESIDENT: h->opt_resident = value < 0 ? 0 : (value > 2 ? 2 : value); break;
     case CORR_OPT_MIX: h->opt_mix = value ? 1 : 0; break;
     case CORR_OPT_UNITS:
       if (value < 0) return fail(CORR_EINVAL, "corr_set_option: CORR_OPT_UNITS must be >= 0");

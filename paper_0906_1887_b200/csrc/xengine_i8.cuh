@@ -67,7 +67,7 @@ struct I8Params {
   int out_shift;     // 8 for 4-bit input (operands are 16 x the samples), else 0
   int accumulate;    // 1: add this integration into d_vis instead of overwriting it
   int mix_full, mix_cut, mix_len;  // diag plans with more groups than CTAs: whole groups + sliced left-over groups (decode_item)
-  int resident;      // 1: CTA pairs keep their A panel of the WHOLE integration in shared memory (T <= 1024) and walk all
+  int resident;      // 1: CTA pairs keep their A panel of the WHOLE integration in shared memory (T <= 1152) and walk all
                      //    column tiles of a row pair with it; an item is then a unit of two row pairs (xengine_i8_resident.cuh)
   int a_sub;         // resident: 128-row sub-stages of the A region (ceil(T / 128))
   int collect;       // 1: 512-wide pair tiles issue their two MMAs per k-step with A-collector reuse

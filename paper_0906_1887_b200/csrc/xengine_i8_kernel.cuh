@@ -66,7 +66,7 @@ __device__ __forceinline__ void xengine_i8_body(const CUtensorMap *maps, int2 *c
   extern __shared__ __align__(1024) uint8_t smem[];
   // 4-bit packed input (kPacked): TMA lands the packed boxes in a second ring (half the bytes) behind the
   // int8 ring; eight expand warps sign-extend the nibbles into the int8 ring in the MN-major SW128 layout.
-  // Resident-A plans (CTA pairs, T <= 1024) put the A panel of the whole integration in front of the ring.
+  // Resident-A plans (CTA pairs, T <= 1152) put the A panel of the whole integration in front of the ring.
   const uint32_t a_bytes = (kPair && p.resident) ? static_cast<uint32_t>(p.a_sub) * kResSubBytes : 0;
   uint8_t *ring_base = smem + a_bytes;
   const uint32_t raw_stage_bytes = kPacked ? static_cast<uint32_t>(p.stage_bytes) / 2 : 0;

@@ -4,7 +4,7 @@
 // shared-memory datapath, not by the tensor pipe: per 256 x 256 tile and k-step a CTA's MMA reads 8 KB of
 // operands, TMA writes 8 KB of new operands, and the epilogue moves another 3.5 x its 64 KB of output per tile
 // (DESIGN.md section 7).  The A operand of a CTA -- its 128-row panel over the WHOLE integration, 128 B x T
-// <= 128 KB -- fits in shared memory when T <= 1024, so a pair keeps it there and walks every column tile of its
+// <= 128 KB -- fits in shared memory when T <= 1152 (144 KB, beside a 3-stage B ring; 4 stages up to T = 1024), so a pair keeps it there and walks every column tile of its
 // row pair with it: A is written to shared memory once per ROW (R + 1 tiles) instead of once per tile, the
 // diagonal tile (whose B operand is the A panel itself) loads nothing at all, and the L2 -> SM traffic of c4
 // drops from 2 x 128 KB to (128 + 128 / 4.5) KB per tile on average.
@@ -20,7 +20,7 @@
 
 namespace corr {
 
-constexpr int kResMaxSub = 8;            // 8 x 128 = 1024 time rows at most
+constexpr int kResMaxSub = 9;            // 9 x 128 = 1152 time rows at most (a 3-stage B ring fits beside them)
 constexpr int kResSubBytes = 128 * 128;  // one sub-stage / one ring stage: 128 time rows of a 128-byte panel
 
 __device__ __forceinline__ void resident_producer(const I8Params &p, const CUtensorMap *maps, uint8_t *smem, uint32_t a_bytes,

@@ -61,7 +61,7 @@ def _cases():
             dtype, N, T, C = ("ci8", "ci4")[k // 24], (64, 32)[k // 24], int(rng.integers(60000, 65536)), int(rng.integers(1, 4))
         opts = []
         if dtype != "cf32":
-            for name, values in (("CORR_OPT_PAIRS", (0, 1, 2)), ("CORR_OPT_WIDE", (0, 1, 2)), ("CORR_OPT_RESIDENT", (0, 1)),
+            for name, values in (("CORR_OPT_PAIRS", (0, 1, 2)), ("CORR_OPT_WIDE", (0, 1, 2)), ("CORR_OPT_RESIDENT", (0, 1, 2)),
                                  ("CORR_OPT_MIX", (0, 1)), ("CORR_OPT_COLLECT", (0, 1)), ("CORR_OPT_PDL", (0, 1, 2)),
                                  ("CORR_OPT_UNITS", (0, 7, 40))):
                 if rng.random() < 0.3:

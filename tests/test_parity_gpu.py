@@ -72,8 +72,11 @@ CI8_SHAPES = [(64, 3, 100), (64, 5, 1), (64, 2, 31), (64, 2, 32), (64, 2, 33), (
               (256, 3, 2100), (320, 1, 2050), (512, 1, 2081),
               # resident-A plans (N_I >= 512, T <= 1024): full-length A region, ragged last sub-stage, odd panel count
               (512, 2, 1000), (640, 3, 1024), (576, 5, 129), (1024, 2, 300),
-              # CTA pairs without the resident plan: 1024 < T < 2048
-              (512, 1, 1100),
+              # CTA pairs without the resident plan: 1152 < T < 2048
+              (512, 1, 1200),
+              # round 3: resident plan up to T = 1152 (9 sub-stages, 3-stage ring) for 4 / 6 / 8 panels per channel, ragged last
+              # sub-stage; 5 / 7 panels (N_I = 320, 448) back on single-CTA slabs; 9 panels streaming above T = 1024
+              (256, 3, 1100), (384, 2, 1152), (512, 2, 1150), (320, 2, 1000), (448, 2, 700), (576, 1, 1100),
               # the largest N_I the ABI admits (528 schedule kinds per channel)
               (4096, 1, 40)]
 

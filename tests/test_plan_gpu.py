@@ -44,6 +44,35 @@ def test_plan_info_names_the_kernel_of_the_paper_shaped_configs(pkg, dtype, N, C
     pkg.corr_destroy(h)
 
 
+@pytest.mark.parametrize("N,T,kid", [
+    (256, 1024, 2), (256, 1152, 2), (256, 1153, 0), (384, 1100, 2), (512, 1152, 2), (512, 1153, 1),   # 4 / 6 / 8 panels: to T = 1152
+    (320, 1000, 0), (288, 500, 0), (448, 1000, 0), (416, 300, 0),                                     # 5 / 7 panels: slabs
+    (576, 1024, 2), (576, 1100, 1), (1024, 1000, 2), (1024, 1100, 1)])                                # >= 9 panels: to T = 1024
+def test_resident_plan_is_taken_where_it_was_measured_to_pay(pkg, N, T, kid):
+    """DESIGN.md section 11 (round 3): thresholds of the resident-A plan, and CORR_OPT_RESIDENT = 2 / 0 around them."""
+    h = pkg.corr_create(N, 3, T, "ci8")
+    assert h.plan_info()["kernel_id"] == kid, h.plan_info()
+    h.set_option(pkg.CORR_OPT_RESIDENT, 2)
+    assert h.plan_info()["kernel_id"] == (2 if T <= 1152 else kid)
+    h.set_option(pkg.CORR_OPT_RESIDENT, 0)
+    assert h.plan_info()["kernel_id"] != 2
+    pkg.corr_destroy(h)
+
+
+@pytest.mark.parametrize("N,C,T", [(320, 2, 1100), (448, 1, 1152), (1024, 1, 1130), (256, 2, 1025)])
+def test_forced_resident_plan_is_bit_exact(pkg, N, C, T):
+    h = pkg.corr_create(N, C, T, "ci8")
+    h.set_option(pkg.CORR_OPT_RESIDENT, 2)
+    assert h.plan_info()["resident"]
+    x = _x(N, C, T, seed=N + T)
+    vis = h.empty_vis()
+    vis.fill_(-0x55555555)
+    pkg.corr_xengine(h, torch.from_numpy(x).cuda(), vis)
+    torch.cuda.synchronize()
+    assert np.array_equal(vis.cpu().numpy(), oracle.xengine_ci8(x, threads=oracle.host_threads()))
+    pkg.corr_destroy(h)
+
+
 def test_plan_info_argument_errors(pkg):
     L = pkg.lib()
     h = pkg.corr_create(32, 4, 50, "ci8")
